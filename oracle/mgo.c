@@ -1,0 +1,454 @@
+/* mgo.c -- CPU oracle (test infrastructure; see mgo.h for scope, citations and pins).
+ *
+ * Plain triple loops, fp64, one code path for all levels (explicit minus-face arrays
+ * on every level).  Expression trees follow SURVEY.md §8(c) C1-C9 / DESIGN.md §3
+ * literally; compile with -ffp-contract=off so that only the fma() calls written
+ * here are fused.  OpenMP, when enabled, only splits the k loop of loops whose
+ * iterations are independent (one colour of a half-sweep, residual, transfers), so
+ * every field is bit-identical to the single-thread run; sums are accumulated per
+ * k-plane in long double and then added in plane order (thread-count independent).
+ */
+#include "mgo.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define MGO_MAX_LEVELS 32
+
+typedef struct {
+    int nx, ny, nz;
+    double h, h2, ih2;          /* C1 */
+    double *bx, *by, *bz;       /* minus-face coefficients */
+    double *p, *f;              /* levels >= 1: correction e and restricted rhs */
+    double *r;                  /* residual scratch (levels that have a coarser one) */
+} level_t;
+
+struct mgo_solver {
+    int nlev;
+    int bc[3];
+    int nu1, nu2, coarse_sweeps;
+    level_t lv[MGO_MAX_LEVELS];
+};
+
+static int g_threads = 0; /* 0 = library default */
+
+int mgo_threads(void)
+{
+#ifdef _OPENMP
+    return g_threads > 0 ? g_threads : omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void mgo_set_threads(int n)
+{
+    g_threads = n;
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#endif
+}
+
+static size_t lv_cells(const level_t *L) { return (size_t)L->nx * L->ny * L->nz; }
+
+#define IDX(L, i, j, k) ((size_t)(i) + (size_t)(L)->nx * ((size_t)(j) + (size_t)(L)->ny * (size_t)(k)))
+
+/* ------------------------------------------------------------------ create */
+int mgo_create(int nx, int ny, int nz, double h, const int bc[3], mgo_solver **out)
+{
+    if (!out || !bc) return MGO_EINVAL;
+    *out = NULL;
+    if (nx < 4 || ny < 4 || nz < 4 || (nx & 1) || (ny & 1) || (nz & 1)) return MGO_EINVAL;
+    if (!(h > 0.0) || !isfinite(h)) return MGO_EINVAL;
+    for (int a = 0; a < 3; ++a)
+        if (bc[a] != 0 && bc[a] != 1) return MGO_EINVAL;
+
+    mgo_solver *s = (mgo_solver *)calloc(1, sizeof(*s));
+    if (!s) return MGO_ENOMEM;
+    memcpy(s->bc, bc, sizeof(s->bc));
+    s->nu1 = 2; s->nu2 = 2; s->coarse_sweeps = 32;
+
+    /* R7: halve every axis while the halved dims stay even (so red-black colouring is
+     * consistent across a periodic wrap on every level) and the smallest dim is > 4. */
+    int n[3] = { nx, ny, nz };
+    double hl = h;
+    int l = 0;
+    for (;;) {
+        level_t *L = &s->lv[l];
+        L->nx = n[0]; L->ny = n[1]; L->nz = n[2];
+        L->h = hl; L->h2 = hl * hl; L->ih2 = 1.0 / L->h2;
+        ++l;
+        int mn = n[0] < n[1] ? n[0] : n[1]; if (n[2] < mn) mn = n[2];
+        if (mn <= 4 || (n[0] % 4) || (n[1] % 4) || (n[2] % 4) || l == MGO_MAX_LEVELS) break;
+        n[0] /= 2; n[1] /= 2; n[2] /= 2; hl *= 2.0;
+    }
+    s->nlev = l;
+    for (l = 0; l < s->nlev; ++l) {
+        level_t *L = &s->lv[l];
+        size_t N = lv_cells(L);
+        L->bx = (double *)malloc(N * sizeof(double));
+        L->by = (double *)malloc(N * sizeof(double));
+        L->bz = (double *)malloc(N * sizeof(double));
+        if (l > 0) {
+            L->p = (double *)malloc(N * sizeof(double));
+            L->f = (double *)malloc(N * sizeof(double));
+        }
+        if (l < s->nlev - 1) L->r = (double *)malloc(N * sizeof(double));
+        if (!L->bx || !L->by || !L->bz || (l > 0 && (!L->p || !L->f)) ||
+            (l < s->nlev - 1 && !L->r)) { mgo_destroy(s); return MGO_ENOMEM; }
+    }
+    /* default density rho == 1 */
+    {
+        level_t *L = &s->lv[0];
+        size_t N = lv_cells(L);
+        double *one = (double *)malloc(N * sizeof(double));
+        if (!one) { mgo_destroy(s); return MGO_ENOMEM; }
+        for (size_t c = 0; c < N; ++c) one[c] = 1.0;
+        mgo_set_density(s, one);
+        free(one);
+    }
+    *out = s;
+    return MGO_OK;
+}
+
+void mgo_destroy(mgo_solver *s)
+{
+    if (!s) return;
+    for (int l = 0; l < s->nlev; ++l) {
+        free(s->lv[l].bx); free(s->lv[l].by); free(s->lv[l].bz);
+        free(s->lv[l].p); free(s->lv[l].f); free(s->lv[l].r);
+    }
+    free(s);
+}
+
+int mgo_set_cycle(mgo_solver *s, int nu1, int nu2, int coarse_sweeps)
+{
+    if (!s || nu1 < 0 || nu2 < 0 || coarse_sweeps < 1) return MGO_EINVAL;
+    s->nu1 = nu1; s->nu2 = nu2; s->coarse_sweeps = coarse_sweeps;
+    return MGO_OK;
+}
+
+/* ------------------------------------------------------------ coefficients */
+int mgo_set_density(mgo_solver *s, const double *rho)
+{
+    if (!s || !rho) return MGO_EINVAL;
+    level_t *L = &s->lv[0];
+    const int nx = L->nx, ny = L->ny, nz = L->nz;
+    size_t N = lv_cells(L);
+    for (size_t c = 0; c < N; ++c)
+        if (!(rho[c] > 0.0) || !isfinite(rho[c])) return MGO_EINVAL;
+
+    /* C2: a = 0.5/rho per cell; face between cells c and nb: beta = a[c] + a[nb];
+     * Neumann wall face: beta = +0.0.  (R4: beta = 1/rho_face, rho_face harmonic mean) */
+    double *a = (double *)malloc(N * sizeof(double));
+    if (!a) return MGO_ENOMEM;
+    for (size_t c = 0; c < N; ++c) a[c] = 0.5 / rho[c];
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                size_t c = IDX(L, i, j, k);
+                int im = i == 0 ? nx - 1 : i - 1;
+                int jm = j == 0 ? ny - 1 : j - 1;
+                int km = k == 0 ? nz - 1 : k - 1;
+                L->bx[c] = (s->bc[0] == 1 && i == 0) ? 0.0 : a[c] + a[IDX(L, im, j, k)];
+                L->by[c] = (s->bc[1] == 1 && j == 0) ? 0.0 : a[c] + a[IDX(L, i, jm, k)];
+                L->bz[c] = (s->bc[2] == 1 && k == 0) ? 0.0 : a[c] + a[IDX(L, i, j, km)];
+            }
+    free(a);
+
+    /* C3 (R8): coarse face = arithmetic mean of the 4 finer faces lying on it */
+    for (int l = 1; l < s->nlev; ++l) {
+        const level_t *F = &s->lv[l - 1];
+        level_t *C = &s->lv[l];
+#pragma omp parallel for schedule(static)
+        for (int K = 0; K < C->nz; ++K)
+            for (int J = 0; J < C->ny; ++J)
+                for (int I = 0; I < C->nx; ++I) {
+                    const int i = 2 * I, j = 2 * J, k = 2 * K;
+                    size_t c = IDX(C, I, J, K);
+                    C->bx[c] = 0.25 * ((F->bx[IDX(F, i, j, k)] + F->bx[IDX(F, i, j + 1, k)]) +
+                                       (F->bx[IDX(F, i, j, k + 1)] + F->bx[IDX(F, i, j + 1, k + 1)]));
+                    C->by[c] = 0.25 * ((F->by[IDX(F, i, j, k)] + F->by[IDX(F, i + 1, j, k)]) +
+                                       (F->by[IDX(F, i, j, k + 1)] + F->by[IDX(F, i + 1, j, k + 1)]));
+                    C->bz[c] = 0.25 * ((F->bz[IDX(F, i, j, k)] + F->bz[IDX(F, i + 1, j, k)]) +
+                                       (F->bz[IDX(F, i, j + 1, k)] + F->bz[IDX(F, i + 1, j + 1, k)]));
+                }
+    }
+    return MGO_OK;
+}
+
+/* ------------------------------------------------------------- the stencil */
+/* C4: neighbour sum S and diagonal D of cell (i,j,k), order x-,x+,y-,y+,z-,z+ */
+static inline void stencil(const level_t *L, const double *p, int i, int j, int k,
+                           double *S, double *D)
+{
+    const int nx = L->nx, ny = L->ny, nz = L->nz;
+    const int im = i == 0 ? nx - 1 : i - 1, ip = i == nx - 1 ? 0 : i + 1;
+    const int jm = j == 0 ? ny - 1 : j - 1, jp = j == ny - 1 ? 0 : j + 1;
+    const int km = k == 0 ? nz - 1 : k - 1, kp = k == nz - 1 ? 0 : k + 1;
+    const double bxm = L->bx[IDX(L, i, j, k)], bxp = L->bx[IDX(L, ip, j, k)];
+    const double bym = L->by[IDX(L, i, j, k)], byp = L->by[IDX(L, i, jp, k)];
+    const double bzm = L->bz[IDX(L, i, j, k)], bzp = L->bz[IDX(L, i, j, kp)];
+    const double pxm = p[IDX(L, im, j, k)], pxp = p[IDX(L, ip, j, k)];
+    const double pym = p[IDX(L, i, jm, k)], pyp = p[IDX(L, i, jp, k)];
+    const double pzm = p[IDX(L, i, j, km)], pzp = p[IDX(L, i, j, kp)];
+    *S = fma(bzp, pzp, fma(bzm, pzm, fma(byp, pyp, fma(bym, pym, fma(bxp, pxp, bxm * pxm)))));
+    *D = ((((bxm + bxp) + bym) + byp) + bzm) + bzp;
+}
+
+static void smooth_half(const level_t *L, int colour, const double *f, double *p)
+{
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < L->nz; ++k)
+        for (int j = 0; j < L->ny; ++j)
+            for (int i = (j + k + colour) & 1; i < L->nx; i += 2) {
+                double S, D;
+                stencil(L, p, i, j, k, &S, &D);
+                const double invD = 1.0 / D;                       /* C5 */
+                p[IDX(L, i, j, k)] = fma(-L->h2, f[IDX(L, i, j, k)], S) * invD;
+            }
+}
+
+/* R9: one sweep = red (colour 0) half-sweep, then black (colour 1) */
+static void sweep(const level_t *L, const double *f, double *p)
+{
+    smooth_half(L, 0, f, p);
+    smooth_half(L, 1, f, p);
+}
+
+static void residual(const level_t *L, const double *f, const double *p, double *r)
+{
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < L->nz; ++k)
+        for (int j = 0; j < L->ny; ++j)
+            for (int i = 0; i < L->nx; ++i) {
+                double S, D;
+                stencil(L, p, i, j, k, &S, &D);
+                size_t c = IDX(L, i, j, k);
+                r[c] = fma(-L->ih2, fma(-D, p[c], S), f[c]);       /* C6 */
+            }
+}
+
+static void apply(const level_t *L, const double *p, double *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < L->nz; ++k)
+        for (int j = 0; j < L->ny; ++j)
+            for (int i = 0; i < L->nx; ++i) {
+                double S, D;
+                stencil(L, p, i, j, k, &S, &D);
+                size_t c = IDX(L, i, j, k);
+                out[c] = L->ih2 * fma(-D, p[c], S);
+            }
+}
+
+/* C7 (R11): coarse rhs = mean of the 8 children */
+static void restrict8(const level_t *F, const level_t *C, const double *r, double *fc)
+{
+#pragma omp parallel for schedule(static)
+    for (int K = 0; K < C->nz; ++K)
+        for (int J = 0; J < C->ny; ++J)
+            for (int I = 0; I < C->nx; ++I) {
+                const int i = 2 * I, j = 2 * J, k = 2 * K;
+                const double r000 = r[IDX(F, i, j, k)],         r100 = r[IDX(F, i + 1, j, k)];
+                const double r010 = r[IDX(F, i, j + 1, k)],     r110 = r[IDX(F, i + 1, j + 1, k)];
+                const double r001 = r[IDX(F, i, j, k + 1)],     r101 = r[IDX(F, i + 1, j, k + 1)];
+                const double r011 = r[IDX(F, i, j + 1, k + 1)], r111 = r[IDX(F, i + 1, j + 1, k + 1)];
+                fc[IDX(C, I, J, K)] =
+                    0.125 * (((r000 + r100) + (r010 + r110)) + ((r001 + r101) + (r011 + r111)));
+            }
+}
+
+static inline double lerp(double near, double far) { return fma(0.25, far, 0.75 * near); }
+
+/* neighbour coarse index on the side the fine child leans to; wrap, or clamp (Neumann) */
+static inline int far_index(int I, int side, int n, int neumann)
+{
+    int Ip = I + 2 * side - 1;
+    if (Ip < 0) Ip = neumann ? 0 : n - 1;
+    if (Ip >= n) Ip = neumann ? n - 1 : 0;
+    return Ip;
+}
+
+/* C8 (R12): p += cell-centred trilinear interpolation of e (x first, then y, then z) */
+static void prolong_add(const mgo_solver *s, const level_t *F, const level_t *C,
+                        const double *e, double *p)
+{
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < F->nz; ++k)
+        for (int j = 0; j < F->ny; ++j)
+            for (int i = 0; i < F->nx; ++i) {
+                const int I = i >> 1, J = j >> 1, K = k >> 1;
+                const int Ip = far_index(I, i & 1, C->nx, s->bc[0] == 1);
+                const int Jp = far_index(J, j & 1, C->ny, s->bc[1] == 1);
+                const int Kp = far_index(K, k & 1, C->nz, s->bc[2] == 1);
+                const double v =
+                    lerp(lerp(lerp(e[IDX(C, I, J, K)],   e[IDX(C, Ip, J, K)]),
+                              lerp(e[IDX(C, I, Jp, K)],  e[IDX(C, Ip, Jp, K)])),
+                         lerp(lerp(e[IDX(C, I, J, Kp)],  e[IDX(C, Ip, J, Kp)]),
+                              lerp(e[IDX(C, I, Jp, Kp)], e[IDX(C, Ip, Jp, Kp)])));
+                p[IDX(F, i, j, k)] = p[IDX(F, i, j, k)] + v;
+            }
+}
+
+/* C9: plane-ordered long-double sums */
+static long double sum_planes(const level_t *L, const double *x, int squared)
+{
+    long double *part = (long double *)malloc((size_t)L->nz * sizeof(long double));
+    size_t plane = (size_t)L->nx * L->ny;
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < L->nz; ++k) {
+        long double acc = 0.0L;
+        const double *q = x + plane * (size_t)k;
+        for (size_t c = 0; c < plane; ++c)
+            acc += squared ? (long double)q[c] * (long double)q[c] : (long double)q[c];
+        part[k] = acc;
+    }
+    long double tot = 0.0L;
+    for (int k = 0; k < L->nz; ++k) tot += part[k];
+    free(part);
+    return tot;
+}
+
+/* ------------------------------------------------------------------ cycle */
+static void vcycle(mgo_solver *s, int l, double *p, const double *f)
+{
+    level_t *L = &s->lv[l];
+    if (l == s->nlev - 1) {                                  /* R13 */
+        for (int it = 0; it < s->coarse_sweeps; ++it) sweep(L, f, p);
+        return;
+    }
+    level_t *C = &s->lv[l + 1];
+    for (int it = 0; it < s->nu1; ++it) sweep(L, f, p);
+    residual(L, f, p, L->r);
+    restrict8(L, C, L->r, C->f);
+    memset(C->p, 0, lv_cells(C) * sizeof(double));
+    vcycle(s, l + 1, C->p, C->f);
+    prolong_add(s, L, C, C->p, p);
+    for (int it = 0; it < s->nu2; ++it) sweep(L, f, p);
+}
+
+int mgo_vcycle(mgo_solver *s, const double *rhs, double *p)
+{
+    if (!s || !rhs || !p) return MGO_EINVAL;
+    vcycle(s, 0, p, rhs);
+    return MGO_OK;
+}
+
+static double residual_norm(mgo_solver *s, const double *rhs, const double *p, double *r_out)
+{
+    level_t *L = &s->lv[0];
+    double *r = r_out ? r_out : (double *)malloc(lv_cells(L) * sizeof(double));
+    residual(L, rhs, p, r);
+    double nrm = (double)sqrtl(sum_planes(L, r, 1));          /* R15 */
+    if (!r_out) free(r);
+    return nrm;
+}
+
+int mgo_residual(mgo_solver *s, const double *rhs, const double *p, double *r_or_null,
+                 double *norm2)
+{
+    if (!s || !rhs || !p) return MGO_EINVAL;
+    double nrm = residual_norm(s, rhs, p, r_or_null);
+    if (norm2) *norm2 = nrm;
+    return MGO_OK;
+}
+
+int mgo_solve(mgo_solver *s, const double *rhs, double *p, double rtol, int max_cycles,
+              int *cycles_out, double *relres_out, double *hist)
+{
+    if (!s || !rhs || !p || !(rtol >= 0.0) || max_cycles < 0) return MGO_EINVAL;
+    level_t *L = &s->lv[0];
+    const size_t N = lv_cells(L);
+    /* R6: singular system (all axes periodic/Neumann): the rhs must be mean-free */
+    {
+        long double mean = sum_planes(L, rhs, 0) / (long double)N;
+        long double nrm = sqrtl(sum_planes(L, rhs, 1));
+        if (fabsl(mean) > 1e-12L * (nrm / sqrtl((long double)N))) return MGO_EINCOMPATIBLE;
+    }
+    double r0 = residual_norm(s, rhs, p, NULL);
+    if (hist) hist[0] = r0;
+    if (!isfinite(r0)) return MGO_EDIVERGED;
+    int k = 0, status = MGO_NOT_CONVERGED;
+    double rk = r0;
+    if (r0 <= rtol * r0) status = MGO_OK;                     /* r0 == 0 */
+    while (status != MGO_OK && k < max_cycles) {
+        vcycle(s, 0, p, rhs);
+        ++k;
+        rk = residual_norm(s, rhs, p, NULL);
+        if (hist) hist[k] = rk;
+        if (!isfinite(rk)) { if (cycles_out) *cycles_out = k; return MGO_EDIVERGED; }
+        if (rk <= rtol * r0) status = MGO_OK;
+    }
+    /* zero arithmetic mean, once, at the end (R6) */
+    {
+        double mean = (double)(sum_planes(L, p, 0) / (long double)N);
+        for (size_t c = 0; c < N; ++c) p[c] = p[c] - mean;
+    }
+    if (cycles_out) *cycles_out = k;
+    if (relres_out) *relres_out = r0 > 0.0 ? rk / r0 : 0.0;
+    return status;
+}
+
+/* ------------------------------------------------------- step-level access */
+int mgo_num_levels(const mgo_solver *s) { return s ? s->nlev : MGO_EINVAL; }
+
+int mgo_level_dims(const mgo_solver *s, int level, int dims[3], double *h_level)
+{
+    if (!s || level < 0 || level >= s->nlev) return MGO_EINVAL;
+    if (dims) { dims[0] = s->lv[level].nx; dims[1] = s->lv[level].ny; dims[2] = s->lv[level].nz; }
+    if (h_level) *h_level = s->lv[level].h;
+    return MGO_OK;
+}
+
+int mgo_get_faces(const mgo_solver *s, int level, double *bx, double *by, double *bz)
+{
+    if (!s || level < 0 || level >= s->nlev) return MGO_EINVAL;
+    const level_t *L = &s->lv[level];
+    size_t bytes = lv_cells(L) * sizeof(double);
+    if (bx) memcpy(bx, L->bx, bytes);
+    if (by) memcpy(by, L->by, bytes);
+    if (bz) memcpy(bz, L->bz, bytes);
+    return MGO_OK;
+}
+
+int mgo_apply(const mgo_solver *s, int level, const double *p, double *out)
+{
+    if (!s || level < 0 || level >= s->nlev || !p || !out) return MGO_EINVAL;
+    apply(&s->lv[level], p, out);
+    return MGO_OK;
+}
+
+int mgo_smooth_half(const mgo_solver *s, int level, int colour, const double *f, double *p)
+{
+    if (!s || level < 0 || level >= s->nlev || (colour != 0 && colour != 1) || !f || !p)
+        return MGO_EINVAL;
+    smooth_half(&s->lv[level], colour, f, p);
+    return MGO_OK;
+}
+
+int mgo_residual_level(const mgo_solver *s, int level, const double *f, const double *p, double *r)
+{
+    if (!s || level < 0 || level >= s->nlev || !f || !p || !r) return MGO_EINVAL;
+    residual(&s->lv[level], f, p, r);
+    return MGO_OK;
+}
+
+int mgo_restrict(const mgo_solver *s, int level, const double *r, double *fc)
+{
+    if (!s || level < 0 || level >= s->nlev - 1 || !r || !fc) return MGO_EINVAL;
+    restrict8(&s->lv[level], &s->lv[level + 1], r, fc);
+    return MGO_OK;
+}
+
+int mgo_prolong_add(const mgo_solver *s, int level, const double *e, double *p)
+{
+    if (!s || level < 0 || level >= s->nlev - 1 || !e || !p) return MGO_EINVAL;
+    prolong_add(s, &s->lv[level], &s->lv[level + 1], e, p);
+    return MGO_OK;
+}

@@ -1,0 +1,82 @@
+/* mgo.h -- CPU ORACLE for the variable-density pressure-Poisson multigrid V-cycle.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may load it.  It shares no code,
+ * header, table or helper with the CUDA path (paper_2605_30082_b200/csrc, include/mg.h).
+ *
+ * What it computes (citations: BJ = BASELINE.json north_star/configs, P:NNN = PAPER.md
+ * line, Rn / Cn = SURVEY.md 8(c) readings and canonical arithmetic, restated in DESIGN.md):
+ *
+ *   A p = f,  (A p)_c = (1/h^2) * sum_{6 faces} beta_face * (p_nb - p_c)        [BJ; R1]
+ *   the discrete form of  div( (1/rho) grad p ) = div(u*)/dt  implied by P:33-36 eq. 1-2,
+ *   cell-centred on a uniform Cartesian finite-volume grid, dense (i,j,k) arrays
+ *   with x fastest (R3), density per cell by volume-fraction mixing.
+ *   beta_face = 1/rho_face with rho_face the harmonic mean of the two cell densities
+ *             = (0.5/rho_a) + (0.5/rho_b)                                       [BJ; R4, C2]
+ *   per axis: periodic (wrap) or homogeneous Neumann (wall-face beta = 0)       [R5]
+ *   solved by geometric multigrid V(nu1,nu2) cycles: red-black Gauss-Seidel, residual,
+ *   8-child-mean restriction, cell-centred trilinear prolongation + correction,
+ *   coarse faces = mean of the 4 coincident fine faces, 4^3-ish coarsest level
+ *   relaxed with a fixed number of sweeps                                       [BJ; R7-R15]
+ *
+ * It is an iteration, so the oracle follows the algorithm step by step in the order
+ * and with the expression trees C1-C9 (no blocking, fusion or reordering).  Every level
+ * stores explicit minus-face arrays bx,by,bz (bx[i,j,k] = face between (i-1,j,k) and
+ * (i,j,k), wrap; a Neumann axis is a periodic axis whose wrap face is 0).
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): closed-form eigenvalues of sine/cosine
+ * modes, symmetry / zero row+column sums, the layered-medium prefix-sum solution,
+ * second-order convergence on a manufactured solution, a dense direct solve at 8^3,
+ * smoother and transfer invariants, config 1's known solution.
+ * PARITY UNPINNED (conventions with no external pin): R8 (4-face coarse
+ * rule), R13 (coarsest sweep count), R11 (8-child mean among the "full-weighting"
+ * readings), R18 (sphere position in the input recipe).
+ *
+ * All pointers are HOST pointers to dense fp64 arrays, idx = i + nx*(j + ny*k).
+ */
+#ifndef MGO_H
+#define MGO_H
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mgo_solver mgo_solver;
+
+enum { MGO_OK = 0, MGO_NOT_CONVERGED = 1, MGO_EINVAL = -1, MGO_ENOMEM = -2,
+       MGO_EINCOMPATIBLE = -4, MGO_EDIVERGED = -5 };
+
+/* bc[axis]: 0 periodic, 1 homogeneous Neumann.  Density defaults to rho == 1. */
+int  mgo_create(int nx, int ny, int nz, double h, const int bc[3], mgo_solver **out);
+void mgo_destroy(mgo_solver *s);
+int  mgo_set_cycle(mgo_solver *s, int nu1, int nu2, int coarse_sweeps);
+int  mgo_set_density(mgo_solver *s, const double *rho);
+
+int  mgo_vcycle(mgo_solver *s, const double *rhs, double *p);
+int  mgo_residual(mgo_solver *s, const double *rhs, const double *p, double *r_or_null,
+                  double *norm2);
+int  mgo_solve(mgo_solver *s, const double *rhs, double *p, double rtol, int max_cycles,
+               int *cycles_out, double *relres_out, double *hist_or_null);
+
+/* ---- step-level entry points (used by the pins and by step-by-step parity) ---- */
+int  mgo_num_levels(const mgo_solver *s);
+int  mgo_level_dims(const mgo_solver *s, int level, int dims[3], double *h_level);
+/* copies the minus-face coefficient arrays of `level` (each nx*ny*nz of that level) */
+int  mgo_get_faces(const mgo_solver *s, int level, double *bx, double *by, double *bz);
+/* out = A_level p */
+int  mgo_apply(const mgo_solver *s, int level, const double *p, double *out);
+/* one half-sweep on cells with (i+j+k)&1 == colour, in place (C4, C5) */
+int  mgo_smooth_half(const mgo_solver *s, int level, int colour, const double *f, double *p);
+/* r = f - A_level p (C6) */
+int  mgo_residual_level(const mgo_solver *s, int level, const double *f, const double *p, double *r);
+/* fc = 8-child mean of r (C7); r on `level`, fc on level+1 */
+int  mgo_restrict(const mgo_solver *s, int level, const double *r, double *fc);
+/* p += P e (C8); p on `level`, e on level+1 */
+int  mgo_prolong_add(const mgo_solver *s, int level, const double *e, double *p);
+/* number of OpenMP threads the loops use (1 if built without OpenMP) */
+int  mgo_threads(void);
+void mgo_set_threads(int n);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
