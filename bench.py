@@ -1,0 +1,372 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement of the B200 multigrid pressure solver.
+
+Step  = one pass of the whole hot path on one batch of synthetic
+        input: mg_set_density(rho) + mg_solve(rhs, p0 = 0) to rtol on the 512^3 drop-film
+        workload (BASELINE.json configs[3], "config 4": the paper's per-device load,
+        PAPER.md:196/218), V(3,3), 8 levels.
+value = fine-grid smoother cell updates per second, N * (nu1+nu2) * cycles / t_step
+        [Gcell-updates/s], inputs resident in HBM, whole-step time in the denominator
+        (norm passes, coefficient setup and mean removal included).
+Also on the line: time-to-rtol, the time of one bare V-cycle (graph replay) with its
+Gcell-updates/s and fraction of the B_sched HBM roofline, the roofline of the dominant
+kernel (level-0 sweep) timed with CUDA events, the same metric end to end from host
+buffers (mg_solve_host), and the CPU oracle on a bounded sample.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload config4]
+
+N > 1 (torchrun): the path does not shard (replicas only); every rank solves
+its own replica, value = total units / max-over-ranks time ("scaling": "weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "V-cycle Gcell-updates/s (time-to-rtol 1e-8 at 512^3 fp64; % HBM roofline alongside)"
+UNIT = "Gcell-updates/s"
+
+# algorithmic HBM bytes: level-0 sweep pass 32 B/cell
+# (p read+write, f, a); coarse-level pass 48 B/cell; whole V(3,3) cycle per fine cell:
+B_SWEEP_L0 = 32.0
+
+
+def b_sched_per_fine_cell(nu1, nu2):
+    """SURVEY §8(d) B_sched: nu1 sweeps in one pass + residual/restrict + prolong/correct/
+    first post-sweep + remaining post-sweeps in one pass; coarse levels 5 arrays."""
+    l0 = 32.0 + 25.0 + 33.0 + (32.0 if nu2 > 1 else 0.0)
+    lc = 48.0 + 41.0 + 49.0 + (48.0 if nu2 > 1 else 0.0)
+    return l0 + lc / 7.0
+
+
+def b_sweep_per_fine_cell(nu1, nu2):
+    l0 = 32.0 * (nu1 + nu2) + 25.0 + 17.0
+    lc = 48.0 * (nu1 + nu2) + 41.0 + 17.0
+    return l0 + lc / 7.0
+
+
+def parse_workload(name: str):
+    name = name.lower()
+    if not name.startswith("config"):
+        raise SystemExit("--workload must look like config4 or config3@128")
+    body = name[len("config"):]
+    if "@" in body:
+        c, n = body.split("@")
+        return int(c), int(n)
+    return int(body), None
+
+
+def peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True,
+                                     timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([t.strip() for t in out.split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=6)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for nm, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle as it stands, on the host cores
+# ------------------------------------------------------------------------------------
+def oracle_sample(w, repeats=1):
+    """Bounded sample of the workload on the CPU oracle: set_density + `repeats` x
+    (one V(nu1,nu2) cycle + residual norm).  Returns (seconds per repeat, threads)."""
+    from oracle import mgo
+    from oracle.mgo import Oracle
+
+    o = Oracle(w.n, w.h, w.bc, w.nu1, w.nu2)
+    o.set_density(w.rho)
+    p = np.zeros(o.shape)
+    times = []
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        o.vcycle(w.rhs, p)
+        o.residual(w.rhs, p)
+        times.append(time.perf_counter() - t0)
+    o.close()
+    return times, mgo.threads()
+
+
+def run_reference(args, w, wname):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    # warm-up + timed steps; each step = one V-cycle + norm on the full workload
+    times, thr = oracle_sample(w, repeats=args.warmup + args.steps)
+    t = times[args.warmup:]
+    per = float(np.mean(t))
+    val = w.ncells * (w.nu1 + w.nu2) / per / 1e9
+    sample = f"1 V({w.nu1},{w.nu2}) cycle + 1 residual norm per step on {wname} (of ~12 cycles per solve)"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": per * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wname, "cells": list(w.n), "cycle": f"V({w.nu1},{w.nu2})", "rtol": w.rtol},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": thr, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------
+# CUDA arm
+# ------------------------------------------------------------------------------------
+def run_cuda(args, w, wname):
+    import torch
+
+    import paper_2605_30082_b200 as mgpkg
+    from paper_2605_30082_b200 import binding as B
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    torch.cuda.set_device(local)
+    devname = f"cuda:{local}"
+    N = w.ncells
+    stream = torch.cuda.Stream(device=devname)
+
+    with torch.cuda.stream(stream):
+        g = mgpkg.Multigrid(w.n, w.h, w.bc, w.nu1, w.nu2, stream=stream, device=devname)
+        rho_d = torch.from_numpy(w.rho).to(devname)
+        rhs_d = torch.from_numpy(w.rhs).to(devname)
+        p_d = torch.zeros(g.shape, dtype=torch.float64, device=devname)
+        max_cycles = 60
+
+        def barrier():
+            torch.cuda.synchronize()
+            if dist is not None:
+                dist.barrier()
+            torch.cuda.synchronize()
+
+        def step():
+            g.set_density(rho_d)
+            p_d.zero_()
+            return g.solve(rhs_d, p_d, w.rtol, max_cycles)
+
+        for _ in range(args.warmup):
+            res = step()
+        barrier()
+        l0 = g.stat(B.MG_STAT_KERNEL_LAUNCHES)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with ClockSampler(local) as clocks:
+            ev0.record(stream)
+            cycles_total = 0
+            for _ in range(args.steps):
+                res = step()
+                cycles_total += res[1]
+            ev1.record(stream)
+            barrier()
+        t_ms = ev0.elapsed_time(ev1)
+        launches = g.stat(B.MG_STAT_KERNEL_LAUNCHES) - l0
+        status, cycles, relres, hist = res
+
+        # time-to-rtol: mg_solve alone
+        g.set_density(rho_d)
+        p_d.zero_()
+        torch.cuda.synchronize()
+        ev0.record(stream)
+        g.solve(rhs_d, p_d, w.rtol, max_cycles)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        t_solve_ms = ev0.elapsed_time(ev1)
+
+        # bare V-cycle (graph replay), 20 launches after 3 warm-ups
+        p_d.zero_()
+        for _ in range(3):
+            g.vcycle(rhs_d, p_d)
+        torch.cuda.synchronize()
+        ev0.record(stream)
+        for _ in range(20):
+            g.vcycle(rhs_d, p_d)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        t_vc_ms = ev0.elapsed_time(ev1) / 20
+        launches_per_vcycle = g.stat(B.MG_STAT_LAUNCHES_PER_VCYCLE)
+
+        # dominant kernel: level-0 red-black sweep pass, CUDA events on the launching stream
+        p_d.zero_()
+        for _ in range(3):
+            g.level_smooth(0, 1, rhs_d, p_d)
+        torch.cuda.synchronize()
+        lk0 = g.stat(B.MG_STAT_KERNEL_LAUNCHES)
+        ev0.record(stream)
+        for _ in range(20):
+            g.level_smooth(0, 1, rhs_d, p_d)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        t_sweep_ms = ev0.elapsed_time(ev1) / 20
+        launches_per_sweep = (g.stat(B.MG_STAT_KERNEL_LAUNCHES) - lk0) / 20
+
+        # set_density alone
+        torch.cuda.synchronize()
+        ev0.record(stream)
+        g.set_density(rho_d)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        t_setrho_ms = ev0.elapsed_time(ev1)
+
+        # end to end from pinned host buffers through mg_solve_host
+        rho_h = torch.from_numpy(w.rho).pin_memory()
+        rhs_h = torch.from_numpy(w.rhs).pin_memory()
+        p_h = torch.empty(g.shape, dtype=torch.float64).pin_memory()
+        e2e_steps = max(1, min(args.steps, 3))
+        g.solve_host(rho_h, rhs_h, p_h, w.rtol, max_cycles)          # warm-up (allocates staging)
+        barrier()
+        ev0.record(stream)
+        e2e_cycles = 0
+        for _ in range(e2e_steps):
+            e2e_cycles += g.solve_host(rho_h, rhs_h, p_h, w.rtol, max_cycles)[1]
+        ev1.record(stream)
+        barrier()
+        t_e2e_ms = ev0.elapsed_time(ev1)
+
+    # max over ranks
+    times = torch.tensor([t_ms, t_e2e_ms], dtype=torch.float64, device=devname)
+    counts = torch.tensor([float(cycles_total), float(e2e_cycles)], dtype=torch.float64, device=devname)
+    if dist is not None:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+        dist.all_reduce(counts, op=dist.ReduceOp.SUM)
+    t_ms, t_e2e_ms = times.tolist()
+    cycles_all, e2e_cycles_all = counts.tolist()
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    upd = w.nu1 + w.nu2
+    value = N * upd * cycles_all / (t_ms * 1e-3) / 1e9
+    e2e_value = N * upd * e2e_cycles_all / (t_e2e_ms * 1e-3) / 1e9
+    peak, peak_src = peaks()
+    sweep_bytes = B_SWEEP_L0 * N
+    achieved = sweep_bytes / (t_sweep_ms * 1e-3) / 1e9
+    bs = b_sched_per_fine_cell(w.nu1, w.nu2) * N
+    bw = b_sweep_per_fine_cell(w.nu1, w.nu2) * N
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": t_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wname, "cells": list(w.n), "bc": list(w.bc), "cycle": f"V({w.nu1},{w.nu2})",
+                   "rtol": w.rtol, "levels": g.num_levels, "cycles_per_solve": cycles, "relres": relres,
+                   "step": "mg_set_density + mg_solve from p=0", "l2": "inputs larger than L2 "
+                   f"({3 * N * 8 / 1e6:.0f} MB resident vs 126 MB)", "parallelism": "replicas only"},
+        "time_to_rtol_ms": t_solve_ms, "set_density_ms": t_setrho_ms,
+        "vcycle": {"ms": t_vc_ms, "gcell_updates_per_s": N * upd / (t_vc_ms * 1e-3) / 1e9,
+                   "launches": launches_per_vcycle,
+                   "frac_of_B_sched_roofline": (bs / (peak * 1e9)) / (t_vc_ms * 1e-3),
+                   "frac_of_B_sweep_roofline": (bw / (peak * 1e9)) / (t_vc_ms * 1e-3),
+                   "B_sched_bytes": bs, "B_sweep_bytes": bw},
+        "roofline": {"bound": "hbm", "kernel": "level-0 red-black sweep pass", "achieved": achieved,
+                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "peak_source": peak_src, "bytes_per_launch": sweep_bytes,
+                     "ms_per_sweep": t_sweep_ms, "launches_per_sweep": launches_per_sweep},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * N * 8, "d2h_bytes_per_step": N * 8,
+                "ms_per_step": t_e2e_ms / e2e_steps, "steps": e2e_steps, "api": "mg_solve_host (pinned host buffers)"},
+        "gpu_launches": int(launches),
+        "clocks": clocks.summary(),
+    }
+    traffic_file = ROOT / "profiles" / "traffic.json"
+    if traffic_file.exists():
+        try:
+            line["roofline"]["traffic"] = json.loads(traffic_file.read_text()).get(wname)
+        except Exception:
+            pass
+    if world == 1 and not args.no_cpu_baseline:
+        times_o, thr = oracle_sample(w, repeats=1)
+        line["cpu_baseline"] = {
+            "value": N * upd / times_o[0] / 1e9, "unit": UNIT, "cores": thr, "kind": "oracle",
+            "sample": f"1 V({w.nu1},{w.nu2}) cycle + 1 residual norm of {wname} ({times_o[0]:.1f} s; a solve is {cycles} cycles)"}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="config4", help="config<k>[@n], k = 1..5 (BASELINE.json configs)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "cuda":
+        args.warmup = 3
+    from workloads import make_workload
+
+    cfg, n = parse_workload(args.workload)
+    rank = int(os.environ.get("RANK", "0"))
+    if args.impl == "reference" and rank != 0:
+        return
+    w = make_workload(cfg, n)
+    wname = f"config{cfg}: {w.n[0]}^3 " + w.note
+    if args.impl == "reference":
+        run_reference(args, w, wname)
+    else:
+        run_cuda(args, w, wname)
+
+
+if __name__ == "__main__":
+    main()

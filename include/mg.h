@@ -1,0 +1,162 @@
+/* mg.h -- C ABI of libmg: B200 (sm_100a) geometric-multigrid solver for the
+ * variable-density pressure Poisson equation of a two-phase VOF projection method,
+ *
+ *      div( (1/rho) grad p ) = div(u*) / dt                 (fp64, one GPU)
+ *
+ * i.e. the pressure step implied by the incompressible Navier-Stokes equations the
+ * paper solves with FS3D (eq. 1-2) on a uniform Cartesian finite-volume
+ * mesh, with cell density from volume-fraction mixing (PAPER.md:47-52,
+ * eq. 5) and "the Multigrid" as the solver.  The paper gives no
+ * further detail; the operation is fixed by BASELINE.json `north_star` and the readings
+ * R1-R19 / expression trees C1-C9 listed in DESIGN.md §3.
+ * The call list is north_star's: mg_create(nx,ny,nz,h,bc), mg_set_density(rho),
+ * mg_vcycle, mg_residual, mg_solve(rhs,p,rtol,max_cycles).
+ *
+ * Discrete problem.  Cell-centred unknowns on nx*ny*nz cells of size h; dense arrays,
+ * x fastest, idx = i + nx*(j + ny*k), no ghost layers, no padding.
+ *      (A p)_c = (1/h^2) * sum over the 6 faces of  beta_face * (p_nb - p_c)
+ *      beta_face = 1/rho_face, rho_face = harmonic mean of the two cell densities
+ * Per axis the boundary is periodic (wrap) or homogeneous Neumann (wall-face beta = 0).
+ * A is singular (constants); rhs must be mean-free; mg_solve returns the zero-mean p.
+ * One V(nu1,nu2) cycle = nu1 red-black Gauss-Seidel sweeps (red = even i+j+k first),
+ * residual, 8-child-mean restriction, recursion on the coarse grid from a zero guess,
+ * cell-centred trilinear prolongation + correction, nu2 sweeps.  Coarse levels carry
+ * face coefficients that are the mean of the 4 finer faces lying on each coarse face;
+ * the coarsest level (reached when halving would make a dimension odd or <= 2, 4^3
+ * for all BASELINE configs) is relaxed with `coarse_sweeps` sweeps.
+ *
+ * Conventions.  All functions return an int status: MG_OK (0), MG_NOT_CONVERGED (1) or
+ * a negative error.  No exception crosses the ABI.  A handle is not thread-safe.
+ * Pointers named *_dev are DEVICE pointers (cudaMalloc / torch tensor .data_ptr()) to
+ * fp64 data on the device that was current at mg_create; *_host are HOST pointers.
+ * The library never frees or keeps caller buffers beyond what each call states.  Work
+ * is enqueued on the handle's stream (mg_set_stream); calls that return a host value
+ * synchronise that stream, the others are asynchronous.
+ */
+#ifndef MG_H
+#define MG_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mg_solver mg_handle;
+
+enum {
+    MG_OK = 0,
+    MG_NOT_CONVERGED = 1,   /* mg_solve hit max_cycles; p holds the last iterate          */
+    MG_EINVAL = -1,         /* bad argument (size < 4, odd size, h <= 0, bad bc, rho <= 0) */
+    MG_ENOMEM = -2,         /* device or host allocation failed / workspace too small      */
+    MG_ECUDA = -3,          /* a CUDA call failed; see mg_last_cuda_error()                */
+    MG_EINCOMPATIBLE = -4,  /* singular system and |mean(rhs)| > 1e-12 * ||rhs||_2/sqrt(N)  */
+    MG_EDIVERGED = -5       /* a residual norm became non-finite                           */
+};
+
+enum { MG_BC_PERIODIC = 0, MG_BC_NEUMANN = 1 };
+
+/* mg_set_option keys */
+enum {
+    MG_OPT_KERNELS = 1,     /* 0 = reference kernels (one launch per half-sweep / transfer),
+                               1 = fused streaming kernels (default)                        */
+    MG_OPT_GRAPH = 2,       /* 1 (default) = V-cycle replayed from a captured CUDA graph     */
+    MG_OPT_COARSE_CTA = 3   /* 1 (default) = levels <= 16^3 run in one persistent CTA       */
+};
+
+/* mg_get_stat keys */
+enum {
+    MG_STAT_KERNEL_LAUNCHES = 1,  /* kernels of this library launched so far (graph nodes
+                                     counted per replay)                                    */
+    MG_STAT_WORKSPACE_BYTES = 2,  /* device bytes owned by the handle                      */
+    MG_STAT_LAUNCHES_PER_VCYCLE = 3
+};
+
+/* Bytes of device workspace a solver of this size needs (all levels, all scratch). */
+size_t mg_workspace_bytes(int nx, int ny, int nz);
+
+/* Create a solver.  bc[axis] in {MG_BC_PERIODIC, MG_BC_NEUMANN} for x,y,z (both sides
+ * of an axis share the type).  Builds the level list, allocates ALL storage once
+ * (cf. the paper's memory-pool lesson) with cudaMalloc, sets rho == 1,
+ * V(2,2), 32 coarsest sweeps, stream 0.
+ * Errors: MG_EINVAL (nx,ny,nz < 4 or odd, h <= 0 or non-finite, bad bc), MG_ENOMEM, MG_ECUDA. */
+int mg_create(int nx, int ny, int nz, double h, const int bc[3], mg_handle **out);
+
+/* As mg_create, but all device storage is carved from caller memory `workspace_dev`
+ * (>= mg_workspace_bytes(), 256-byte aligned; e.g. a torch uint8 tensor).  The caller
+ * keeps ownership and must keep it alive until mg_destroy. */
+int mg_create_in(int nx, int ny, int nz, double h, const int bc[3],
+                 void *workspace_dev, size_t workspace_bytes, mg_handle **out);
+
+/* Frees everything the library allocated (never caller buffers).  NULL is allowed. */
+void mg_destroy(mg_handle *s);
+
+/* All later work is enqueued on `cuda_stream` (a cudaStream_t; NULL = default stream). */
+int mg_set_stream(mg_handle *s, void *cuda_stream);
+
+/* V(nu1,nu2) and the number of sweeps on the coarsest level (defaults 2,2,32). */
+int mg_set_cycle(mg_handle *s, int nu1, int nu2, int coarse_sweeps);
+
+int mg_set_option(mg_handle *s, int key, int value);
+int mg_get_stat(const mg_handle *s, int key, long long *value_host);
+
+/* Density field: rho_dev = N doubles, read-only, may be freed once the stream has
+ * passed this call.  The library derives and owns a = 0.5/rho (level 0) and the face
+ * coefficients of every coarser level.  Synchronises the stream (validity check).
+ * MG_EINVAL if any rho is <= 0 or non-finite (coefficients are then unspecified). */
+int mg_set_density(mg_handle *s, const double *rho_dev);
+
+/* One V(nu1,nu2) cycle in place on p_dev for right-hand side rhs_dev (N doubles each).
+ * No mean removal, no norm.  Asynchronous on the stream. */
+int mg_vcycle(mg_handle *s, const double *rhs_dev, double *p_dev);
+
+/* r = rhs - A p.  Writes r to r_dev if non-NULL, and sqrt(sum r^2) to *norm2_host if
+ * non-NULL (then the stream is synchronised). */
+int mg_residual(mg_handle *s, const double *rhs_dev, const double *p_dev,
+                double *r_dev, double *norm2_host);
+
+/* V-cycles until ||rhs - A p||_2 <= rtol * ||rhs - A p_0||_2 or max_cycles.
+ * p_dev: in = initial guess, out = iterate with its arithmetic mean removed.
+ * hist_host (NULL or >= max_cycles+1 doubles) receives ||r_k||_2, k = 0..cycles.
+ * Returns MG_OK, MG_NOT_CONVERGED, MG_EINCOMPATIBLE (p untouched), MG_EDIVERGED.
+ * A residual that rises in the first cycle is normal and not an error. */
+int mg_solve(mg_handle *s, const double *rhs_dev, double *p_dev, double rtol, int max_cycles,
+             int *cycles_host, double *relres_host, double *hist_host);
+
+/* End-to-end variant on HOST buffers (N doubles each; pinned memory makes the copies
+ * asynchronous): copies rhs_host and, if non-NULL, rho_host to the device (then also
+ * runs mg_set_density), solves from the initial guess p = 0, copies the zero-mean
+ * solution to p_host (output only).  Device staging buffers (3 N doubles) are owned by
+ * the handle and allocated on first use.  Same return codes as mg_solve. */
+int mg_solve_host(mg_handle *s, const double *rho_host, const double *rhs_host, double *p_host,
+                  double rtol, int max_cycles, int *cycles_host, double *relres_host,
+                  double *hist_host);
+
+const char *mg_strerror(int status);
+/* Text of the last CUDA error seen by this thread inside the library ("" if none). */
+const char *mg_last_cuda_error(void);
+
+/* ---- introspection and single steps of the cycle (same kernels the cycle uses;
+ *      meant for step-by-step verification and for embedding in other cycles) ---- */
+int mg_num_levels(const mg_handle *s);
+int mg_level_dims(const mg_handle *s, int level, int dims[3], double *h_level_host);
+/* Copies the minus-face coefficients of `level` into caller device arrays (level cells
+ * each): bx[i,j,k] = face between (i-1,j,k) and (i,j,k), etc.; wall faces are 0. */
+int mg_level_faces(mg_handle *s, int level, double *bx_dev, double *by_dev, double *bz_dev);
+/* One Gauss-Seidel half-sweep on the cells with (i+j+k)&1 == colour, in place. */
+int mg_level_smooth_half(mg_handle *s, int level, int colour, const double *f_dev, double *p_dev);
+/* `sweeps` full red-black sweeps with the kernels selected by MG_OPT_KERNELS. */
+int mg_level_smooth(mg_handle *s, int level, int sweeps, const double *f_dev, double *p_dev);
+/* r = f - A_level p */
+int mg_level_residual(mg_handle *s, int level, const double *f_dev, const double *p_dev,
+                      double *r_dev);
+/* fc = 8-child mean of (f - A_level p): fused residual + restriction, level -> level+1 */
+int mg_level_residual_restrict(mg_handle *s, int level, const double *f_dev,
+                               const double *p_dev, double *fc_dev);
+/* p += trilinear prolongation of e (e on level+1, p on level) */
+int mg_level_prolong_add(mg_handle *s, int level, const double *e_dev, double *p_dev);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MG_H */

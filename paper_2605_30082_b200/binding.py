@@ -1,0 +1,234 @@
+"""ctypes binding of libmg: argument marshalling only (include/mg.h has the semantics).
+
+Tensors are torch CUDA fp64 tensors of shape (nz, ny, nx) (x fastest); torch supplies
+device memory and the stream, nothing else.  Every ``mg_*`` entry point of the header
+is reachable as ``lib().mg_*``; :class:`Multigrid` wraps a handle.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+from . import _build
+
+MG_OK, MG_NOT_CONVERGED = 0, 1
+MG_EINVAL, MG_ENOMEM, MG_ECUDA, MG_EINCOMPATIBLE, MG_EDIVERGED = -1, -2, -3, -4, -5
+MG_BC_PERIODIC, MG_BC_NEUMANN = 0, 1
+MG_OPT_KERNELS, MG_OPT_GRAPH, MG_OPT_COARSE_CTA = 1, 2, 3
+MG_STAT_KERNEL_LAUNCHES, MG_STAT_WORKSPACE_BYTES, MG_STAT_LAUNCHES_PER_VCYCLE = 1, 2, 3
+
+_vp, _dp, _ip = C.c_void_p, C.c_void_p, C.POINTER(C.c_int)   # device pointers travel as integers
+_hp = C.POINTER(C.c_double)
+
+SIGNATURES = {
+    "mg_workspace_bytes": (C.c_size_t, [C.c_int, C.c_int, C.c_int]),
+    "mg_create": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_double, _ip, C.POINTER(_vp)]),
+    "mg_create_in": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_double, _ip, _vp, C.c_size_t, C.POINTER(_vp)]),
+    "mg_destroy": (None, [_vp]),
+    "mg_set_stream": (C.c_int, [_vp, _vp]),
+    "mg_set_cycle": (C.c_int, [_vp, C.c_int, C.c_int, C.c_int]),
+    "mg_set_option": (C.c_int, [_vp, C.c_int, C.c_int]),
+    "mg_get_stat": (C.c_int, [_vp, C.c_int, C.POINTER(C.c_longlong)]),
+    "mg_set_density": (C.c_int, [_vp, _dp]),
+    "mg_vcycle": (C.c_int, [_vp, _dp, _dp]),
+    "mg_residual": (C.c_int, [_vp, _dp, _dp, _dp, _hp]),
+    "mg_solve": (C.c_int, [_vp, _dp, _dp, C.c_double, C.c_int, _ip, _hp, _hp]),
+    "mg_solve_host": (C.c_int, [_vp, _vp, _vp, _vp, C.c_double, C.c_int, _ip, _hp, _hp]),
+    "mg_strerror": (C.c_char_p, [C.c_int]),
+    "mg_last_cuda_error": (C.c_char_p, []),
+    "mg_num_levels": (C.c_int, [_vp]),
+    "mg_level_dims": (C.c_int, [_vp, C.c_int, _ip, _hp]),
+    "mg_level_faces": (C.c_int, [_vp, C.c_int, _dp, _dp, _dp]),
+    "mg_level_smooth_half": (C.c_int, [_vp, C.c_int, C.c_int, _dp, _dp]),
+    "mg_level_smooth": (C.c_int, [_vp, C.c_int, C.c_int, _dp, _dp]),
+    "mg_level_residual": (C.c_int, [_vp, C.c_int, _dp, _dp, _dp]),
+    "mg_level_residual_restrict": (C.c_int, [_vp, C.c_int, _dp, _dp, _dp]),
+    "mg_level_prolong_add": (C.c_int, [_vp, C.c_int, _dp, _dp]),
+}
+
+_lib = None
+
+
+def lib():
+    """The loaded libmg (built on demand).  Raises if it cannot be built or loaded."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(str(path))
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)          # AttributeError = header/library mismatch
+            fn.restype, fn.argtypes = res, args
+        L._path = str(path)
+        _lib = L
+    return _lib
+
+
+class MgError(RuntimeError):
+    def __init__(self, code):
+        msg = lib().mg_strerror(code).decode()
+        if code == MG_ECUDA:
+            msg += ": " + lib().mg_last_cuda_error().decode()
+        super().__init__(f"libmg error {code}: {msg}")
+        self.code = code
+
+
+def _chk(code, ok=(MG_OK,)):
+    if code not in ok:
+        raise MgError(code)
+    return code
+
+
+def workspace_bytes(nx, ny, nz):
+    return lib().mg_workspace_bytes(nx, ny, nz)
+
+
+def _ptr(t, shape=None):
+    import torch
+
+    if t is None:
+        return None
+    assert isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous(), \
+        "expected a contiguous CUDA float64 tensor"
+    if shape is not None:
+        assert tuple(t.shape) == tuple(shape), (tuple(t.shape), tuple(shape))
+    return t.data_ptr()
+
+
+class Multigrid:
+    """Handle to one solver.  n = (nx, ny, nz) or a single int; bc per axis (0 periodic,
+    1 Neumann).  Device storage comes from a torch tensor (mg_create_in); the stream is
+    torch's current stream at construction unless ``stream`` is given."""
+
+    def __init__(self, n, h, bc, nu1=2, nu2=2, coarse_sweeps=32, stream=None, device="cuda:0"):
+        import torch
+
+        nx, ny, nz = (n, n, n) if isinstance(n, int) else n
+        self.n = (int(nx), int(ny), int(nz))
+        self.shape = (self.n[2], self.n[1], self.n[0])
+        self.device = torch.device(device)
+        L = lib()
+        self._h = _vp()
+        need = L.mg_workspace_bytes(*self.n)
+        if need == 0:
+            raise MgError(MG_EINVAL)
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
+            base = (self._ws.data_ptr() + 255) // 256 * 256
+            bca = (C.c_int * 3)(*[int(b) for b in bc])
+            _chk(L.mg_create_in(*self.n, float(h), bca, base, need, C.byref(self._h)))
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            _chk(L.mg_set_stream(self._h, self.stream.cuda_stream))
+        _chk(L.mg_set_cycle(self._h, nu1, nu2, coarse_sweeps))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().mg_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- configuration
+    def set_cycle(self, nu1, nu2, coarse_sweeps=32):
+        _chk(lib().mg_set_cycle(self._h, nu1, nu2, coarse_sweeps))
+
+    def set_option(self, key, value):
+        _chk(lib().mg_set_option(self._h, key, value))
+
+    def stat(self, key):
+        v = C.c_longlong()
+        _chk(lib().mg_get_stat(self._h, key, C.byref(v)))
+        return v.value
+
+    @property
+    def num_levels(self):
+        return lib().mg_num_levels(self._h)
+
+    def level_dims(self, level):
+        d = (C.c_int * 3)()
+        h = C.c_double()
+        _chk(lib().mg_level_dims(self._h, level, d, C.byref(h)))
+        return (d[0], d[1], d[2]), h.value
+
+    def level_shape(self, level):
+        (nx, ny, nz), _ = self.level_dims(level)
+        return (nz, ny, nx)
+
+    # ---- the calls of the boundary
+    def set_density(self, rho):
+        _chk(lib().mg_set_density(self._h, _ptr(rho, self.shape)))
+
+    def vcycle(self, rhs, p):
+        _chk(lib().mg_vcycle(self._h, _ptr(rhs, self.shape), _ptr(p, self.shape)))
+        return p
+
+    def residual(self, rhs, p, r=None):
+        nrm = C.c_double()
+        _chk(lib().mg_residual(self._h, _ptr(rhs, self.shape), _ptr(p, self.shape),
+                               _ptr(r, self.shape), C.byref(nrm)))
+        return nrm.value
+
+    def solve(self, rhs, p, rtol, max_cycles):
+        """Returns (status, cycles, relres, hist[0..cycles]); p updated in place."""
+        cyc, rel = C.c_int(), C.c_double()
+        hist = (C.c_double * (max_cycles + 1))()
+        st = lib().mg_solve(self._h, _ptr(rhs, self.shape), _ptr(p, self.shape), float(rtol),
+                            int(max_cycles), C.byref(cyc), C.byref(rel), hist)
+        if st < 0:
+            raise MgError(st)
+        return st, cyc.value, rel.value, list(hist[: cyc.value + 1])
+
+    def solve_host(self, rho_host, rhs_host, p_host, rtol, max_cycles):
+        """Host-buffer variant: CPU torch tensors (ideally pinned) of shape (nz,ny,nx)."""
+        cyc, rel = C.c_int(), C.c_double()
+        hist = (C.c_double * (max_cycles + 1))()
+        for t in (rho_host, rhs_host, p_host):
+            assert t is None or (not t.is_cuda and t.is_contiguous() and tuple(t.shape) == self.shape)
+        st = lib().mg_solve_host(self._h, rho_host.data_ptr() if rho_host is not None else None,
+                                 rhs_host.data_ptr(), p_host.data_ptr(), float(rtol), int(max_cycles),
+                                 C.byref(cyc), C.byref(rel), hist)
+        if st < 0:
+            raise MgError(st)
+        return st, cyc.value, rel.value, list(hist[: cyc.value + 1])
+
+    # ---- single steps
+    def level_faces(self, level):
+        import torch
+
+        shp = self.level_shape(level)
+        out = [torch.empty(shp, dtype=torch.float64, device=self.device) for _ in range(3)]
+        _chk(lib().mg_level_faces(self._h, level, *[_ptr(t) for t in out]))
+        return out
+
+    def level_smooth_half(self, level, colour, f, p):
+        _chk(lib().mg_level_smooth_half(self._h, level, colour, _ptr(f, self.level_shape(level)),
+                                        _ptr(p, self.level_shape(level))))
+        return p
+
+    def level_smooth(self, level, sweeps, f, p):
+        _chk(lib().mg_level_smooth(self._h, level, sweeps, _ptr(f, self.level_shape(level)),
+                                   _ptr(p, self.level_shape(level))))
+        return p
+
+    def level_residual(self, level, f, p):
+        import torch
+
+        r = torch.empty(self.level_shape(level), dtype=torch.float64, device=self.device)
+        _chk(lib().mg_level_residual(self._h, level, _ptr(f, r.shape), _ptr(p, r.shape), _ptr(r)))
+        return r
+
+    def level_residual_restrict(self, level, f, p):
+        import torch
+
+        fc = torch.empty(self.level_shape(level + 1), dtype=torch.float64, device=self.device)
+        shp = self.level_shape(level)
+        _chk(lib().mg_level_residual_restrict(self._h, level, _ptr(f, shp), _ptr(p, shp), _ptr(fc)))
+        return fc
+
+    def level_prolong_add(self, level, e, p):
+        _chk(lib().mg_level_prolong_add(self._h, level, _ptr(e, self.level_shape(level + 1)),
+                                        _ptr(p, self.level_shape(level))))
+        return p

@@ -1,0 +1,248 @@
+"""GPU parity: the CUDA path (through the C ABI of include/mg.h) against the CPU oracle,
+element by element on identical seeded inputs.
+
+Bars (BASELINE.json north_star): fields of single steps and of V-cycles are
+compared BIT-EXACTLY (both sides implement the expression trees C1-C9 with IEEE fp64
+add/mul/fma/div); per-cycle residual norms within relative 1e-10 (the two sides only
+differ in the summation order of the norm); p after the solve within 1e-9 max-abs
+relative (the mean that is subtracted comes from differently ordered sums).
+"""
+import itertools
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle.mgo import Oracle  # noqa: E402
+from workloads import make_workload  # noqa: E402
+
+P, N = 0, 1
+NORM_RTOL = 1e-10
+P_RTOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def mgmod():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2605_30082_b200 as m
+    return m
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+
+
+def host(t):
+    return t.detach().cpu().numpy()
+
+
+def pair(mgmod, n, h, bc, nu=(2, 2), rho=None, coarse_sweeps=32, **opts):
+    o = Oracle(n, h, bc, nu[0], nu[1], coarse_sweeps)
+    g = mgmod.Multigrid(n, h, bc, nu[0], nu[1], coarse_sweeps)
+    from paper_2605_30082_b200 import binding as B
+    for key, name in ((B.MG_OPT_KERNELS, "kernels"), (B.MG_OPT_GRAPH, "graph"), (B.MG_OPT_COARSE_CTA, "coarse_cta")):
+        if name in opts:
+            g.set_option(key, opts[name])
+    if rho is not None:
+        o.set_density(rho)
+        g.set_density(dev(rho))
+    return o, g
+
+
+def random_rho(uniform, seed, shape):
+    return np.exp(uniform(seed, shape, np.log(1.2), np.log(998.0)))
+
+
+SHAPES = [
+    ((32, 32, 32), (P, P, P)),
+    ((32, 32, 32), (P, P, N)),
+    ((48, 32, 24), (N, P, N)),     # non-cubic, coarsest 12x8x6
+    ((40, 24, 56), (P, N, P)),     # ragged against every tile size, single coarsening
+    ((64, 16, 8), (N, N, N)),
+    ((8, 8, 8), (P, P, N)),
+    ((4, 4, 4), (P, P, P)),        # single level
+]
+
+
+# --------------------------------------------------------------------------- #
+# single steps, every level, bit exact
+# --------------------------------------------------------------------------- #
+@pytest.mark.parametrize("n,bc", SHAPES)
+def test_steps_bit_exact(mgmod, uniform, n, bc):
+    h = 1.0 / n[0]
+    rho = random_rho(uniform, 5, (n[2], n[1], n[0]))
+    o, g = pair(mgmod, n, h, bc, rho=rho)
+    assert o.num_levels == g.num_levels
+    for lvl in range(o.num_levels):
+        assert o.level_dims(lvl) == g.level_dims(lvl)
+        shp = o.level_shape(lvl)
+        # coefficients (A0)
+        for bo, bg in zip(o.faces(lvl), g.level_faces(lvl)):
+            assert np.array_equal(bo, host(bg)), f"faces level {lvl}"
+        f, p0 = uniform(10 + lvl, shp), uniform(20 + lvl, shp)
+        # half sweeps (A1/A6), both colours in order
+        po, pg = p0.copy(), dev(p0)
+        fd = dev(f)
+        for colour in (0, 1, 0):
+            o.smooth_half(colour, f, po, lvl)
+            g.level_smooth_half(lvl, colour, fd, pg)
+            assert np.array_equal(po, host(pg)), f"half sweep colour {colour} level {lvl}"
+        # full sweeps through whichever kernels the cycle uses
+        po2, pg2 = p0.copy(), dev(p0)
+        for _ in range(3):
+            o.sweep(f, po2, lvl)
+        g.level_smooth(lvl, 3, fd, pg2)
+        assert np.array_equal(po2, host(pg2)), f"3 sweeps level {lvl}"
+        # residual (A2)
+        assert np.array_equal(o.residual_level(f, po, lvl), host(g.level_residual(lvl, fd, pg)))
+        if lvl < o.num_levels - 1:
+            # residual + restriction (A2+A3)
+            fc_o = o.restrict(o.residual_level(f, po, lvl), lvl)
+            assert np.array_equal(fc_o, host(g.level_residual_restrict(lvl, fd, pg)))
+            # prolongation + correction (A5)
+            e = uniform(30 + lvl, o.level_shape(lvl + 1))
+            o.prolong_add(e, po, lvl)
+            g.level_prolong_add(lvl, dev(e), pg)
+            assert np.array_equal(po, host(pg)), f"prolong level {lvl}"
+
+
+# --------------------------------------------------------------------------- #
+# V-cycles: every kernel-selection combination gives the oracle's iterate bit for bit
+# --------------------------------------------------------------------------- #
+OPTS = [dict(kernels=k, graph=gr, coarse_cta=c) for k, gr, c in itertools.product((0, 1), (0, 1), (0, 1))]
+
+
+@pytest.mark.parametrize("n,bc", SHAPES[:5])
+@pytest.mark.parametrize("opts", OPTS, ids=lambda d: "k%d-g%d-c%d" % (d["kernels"], d["graph"], d["coarse_cta"]))
+@pytest.mark.parametrize("nu", [(2, 2), (3, 3), (1, 0)])
+def test_vcycle_bit_exact(mgmod, uniform, n, bc, opts, nu):
+    h = 1.0 / n[0]
+    shp = (n[2], n[1], n[0])
+    rho = random_rho(uniform, 7, shp)
+    o, g = pair(mgmod, n, h, bc, nu=nu, rho=rho, coarse_sweeps=8, **opts)
+    f = uniform(8, shp)
+    f -= f.mean()
+    po, pg, fd = np.zeros(shp), dev(np.zeros(shp)), dev(f)
+    for cyc in range(3):
+        o.vcycle(f, po)
+        g.vcycle(fd, pg)
+        assert np.array_equal(po, host(pg)), f"cycle {cyc}"
+    assert g.residual(fd, pg) == pytest.approx(o.residual(f, po), rel=NORM_RTOL)
+
+
+# --------------------------------------------------------------------------- #
+# solves on the BASELINE configs (and scaled twins): norms 1e-10, p 1e-9
+# --------------------------------------------------------------------------- #
+def check_solve(mgmod, w, max_cycles=40, **opts):
+    o, g = pair(mgmod, w.n, w.h, w.bc, nu=(w.nu1, w.nu2), rho=w.rho, **opts)
+    po = np.zeros(o.shape)
+    so, co, ro, ho = o.solve(w.rhs, po, w.rtol, max_cycles)
+    pg = dev(np.zeros(o.shape))
+    sg, cg, rg, hg = g.solve(dev(w.rhs), pg, w.rtol, max_cycles)
+    assert (sg, cg) == (so, co)
+    hg = np.array(hg)
+    assert np.abs(hg - ho).max() <= NORM_RTOL * ho[0] and np.all(np.abs(hg / ho - 1) <= NORM_RTOL), (hg, ho)
+    assert rg == pytest.approx(ro, rel=NORM_RTOL)
+    pgh = host(pg)
+    assert np.abs(pgh - po).max() <= P_RTOL * np.abs(po).max()
+    assert abs(pgh.mean()) <= 1e-12 * np.abs(pgh).max()
+    return o, g, po, pgh, ho
+
+
+def test_solve_config1(mgmod):
+    w = make_workload(1)
+    o, g, po, pg, hist = check_solve(mgmod, w)
+    assert len(hist) - 1 <= 12 and np.abs(pg - w.p_exact).max() <= 1e-10
+
+
+@pytest.mark.parametrize("cfg,n", [(2, 64), (2, 128), (3, 64), (3, 128), (5, 128)])
+def test_solve_config_twins(mgmod, cfg, n):
+    check_solve(mgmod, make_workload(cfg, n))
+
+
+@pytest.mark.parametrize("opts", [dict(kernels=0, graph=0, coarse_cta=0), dict(kernels=1, graph=1, coarse_cta=0)],
+                         ids=["reference-kernels", "fused-no-cta"])
+def test_solve_kernel_variants_agree(mgmod, opts):
+    check_solve(mgmod, make_workload(3, 64), **opts)
+
+
+def test_solve_host_buffers(mgmod):
+    w = make_workload(3, 64)
+    o, g = pair(mgmod, w.n, w.h, w.bc, nu=(w.nu1, w.nu2))
+    o.set_density(w.rho)
+    po = np.zeros(o.shape)
+    so, co, ro, ho = o.solve(w.rhs, po, w.rtol, 40)
+    rho_h = torch.from_numpy(w.rho).pin_memory()
+    rhs_h = torch.from_numpy(w.rhs).pin_memory()
+    p_h = torch.empty(o.shape, dtype=torch.float64).pin_memory()
+    sg, cg, rg, hg = g.solve_host(rho_h, rhs_h, p_h, w.rtol, 40)
+    assert (sg, cg) == (so, co)
+    assert np.all(np.abs(np.array(hg) / ho - 1) <= NORM_RTOL)
+    assert np.abs(p_h.numpy() - po).max() <= P_RTOL * np.abs(po).max()
+
+
+# --------------------------------------------------------------------------- #
+# edge cases and error behaviour of the boundary
+# --------------------------------------------------------------------------- #
+def test_error_codes_and_degenerate_inputs(mgmod, uniform):
+    from paper_2605_30082_b200 import binding as B
+    for bad in [((7, 8, 8), 0.1, (P, P, P)), ((8, 8, 2), 0.1, (P, P, P)), ((8, 8, 8), -1.0, (P, P, P)),
+                ((8, 8, 8), 0.1, (P, 3, P))]:
+        with pytest.raises(B.MgError) as ei:
+            mgmod.Multigrid(*bad)
+        assert ei.value.code == B.MG_EINVAL
+    g = mgmod.Multigrid((8, 8, 8), 0.125, (P, P, P))
+    rho = np.ones((8, 8, 8))
+    rho[1, 2, 3] = 0.0
+    with pytest.raises(B.MgError) as ei:
+        g.set_density(dev(rho))
+    assert ei.value.code == B.MG_EINVAL
+    rho[1, 2, 3] = np.nan
+    with pytest.raises(B.MgError):
+        g.set_density(dev(rho))
+    g.set_density(dev(np.ones((8, 8, 8))))
+    f = uniform(3, (8, 8, 8))
+    p = dev(np.full((8, 8, 8), 0.25))
+    with pytest.raises(B.MgError) as ei:
+        g.solve(dev(f + 1.0), p, 1e-8, 5)
+    assert ei.value.code == B.MG_EINCOMPATIBLE
+    assert np.all(host(p) == 0.25)                       # p untouched
+    f -= f.mean()
+    st, cyc, rel, hist = g.solve(dev(f), p, 1e-14, 2)
+    assert st == B.MG_NOT_CONVERGED and cyc == 2 and len(hist) == 3
+    # max_cycles = 0: only the initial residual and the mean removal
+    p = dev(uniform(4, (8, 8, 8)))
+    st, cyc, rel, hist = g.solve(dev(f), p, 1e-8, 0)
+    assert st == B.MG_NOT_CONVERGED and cyc == 0 and len(hist) == 1 and abs(host(p).mean()) < 1e-16
+    # zero right-hand side, zero guess: converged immediately with p = 0
+    z = dev(np.zeros((8, 8, 8)))
+    st, cyc, rel, hist = g.solve(z, dev(np.zeros((8, 8, 8))), 1e-8, 5)
+    assert st == B.MG_OK and cyc == 0 and hist == [0.0]
+    assert g.stat(B.MG_STAT_KERNEL_LAUNCHES) > 0 and g.stat(B.MG_STAT_WORKSPACE_BYTES) > 0
+
+
+def test_default_density_is_one(mgmod, uniform):
+    n = (16, 16, 16)
+    o, g = pair(mgmod, n, 1 / 16, (P, P, N))           # no set_density on either side
+    f = uniform(2, (16, 16, 16))
+    f -= f.mean()
+    po, pg = np.zeros((16, 16, 16)), dev(np.zeros((16, 16, 16)))
+    o.vcycle(f, po)
+    g.vcycle(dev(f), pg)
+    assert np.array_equal(po, host(pg))
+
+
+def test_density_can_be_replaced(mgmod, uniform):
+    w = make_workload(3, 32)
+    o, g = pair(mgmod, w.n, w.h, w.bc, nu=(3, 3), rho=random_rho(uniform, 1, (32, 32, 32)))
+    pg, po = dev(np.zeros(o.shape)), np.zeros(o.shape)
+    g.vcycle(dev(w.rhs), pg)                              # graph captured with the first density
+    o.vcycle(w.rhs, po)
+    o.set_density(w.rho)
+    g.set_density(dev(w.rho))
+    g.vcycle(dev(w.rhs), pg)
+    o.vcycle(w.rhs, po)
+    assert np.array_equal(po, host(pg))
