@@ -126,7 +126,7 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------
 # reference arm / cpu_baseline: the oracle as it stands, on the host cores
 # ------------------------------------------------------------------------------------
-def oracle_sample(w, repeats=1):
+def oracle_sample(w, repeats=1, min_seconds=0.0):
     """Bounded sample of the workload on the CPU oracle: set_density + `repeats` x
     (one V(nu1,nu2) cycle + residual norm).  Returns (seconds per repeat, threads)."""
     from oracle import mgo
@@ -136,7 +136,7 @@ def oracle_sample(w, repeats=1):
     o.set_density(w.rho)
     p = np.zeros(o.shape)
     times = []
-    for _ in range(repeats):
+    while len(times) < repeats or (min_seconds and sum(times) < min_seconds and len(times) < 40):
         t0 = time.perf_counter()
         o.vcycle(w.rhs, p)
         o.residual(w.rhs, p)
@@ -334,10 +334,11 @@ def run_cuda(args, w, wname):
         except Exception:
             pass
     if world == 1 and not args.no_cpu_baseline:
-        times_o, thr = oracle_sample(w, repeats=1)
+        times_o, thr = oracle_sample(w, repeats=1, min_seconds=10.0)
         line["cpu_baseline"] = {
-            "value": N * upd / times_o[0] / 1e9, "unit": UNIT, "cores": thr, "kind": "oracle",
-            "sample": f"1 V({w.nu1},{w.nu2}) cycle + 1 residual norm of {wname} ({times_o[0]:.1f} s; a solve is {cycles} cycles)"}
+            "value": N * upd * len(times_o) / sum(times_o) / 1e9, "unit": UNIT, "cores": thr, "kind": "oracle",
+            "sample": f"{len(times_o)} x (1 V({w.nu1},{w.nu2}) cycle + 1 residual norm) of {wname} "
+                      f"({sum(times_o):.1f} s in total; a solve is {cycles} cycles)"}
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

@@ -64,6 +64,9 @@ SHAPES = [
     ((64, 16, 8), (N, N, N)),
     ((8, 8, 8), (P, P, N)),
     ((4, 4, 4), (P, P, P)),        # single level
+    ((72, 40, 36), (P, N, N)),     # streaming kernels: ragged tiles in x and y, walls in y and z
+    ((64, 64, 64), (N, P, N)),     # streaming kernels on two levels, wall in x
+    ((128, 32, 64), (P, P, P)),    # several x tiles, periodic wrap everywhere
 ]
 
 
@@ -115,7 +118,7 @@ def test_steps_bit_exact(mgmod, uniform, n, bc):
 OPTS = [dict(kernels=k, graph=gr, coarse_cta=c) for k, gr, c in itertools.product((0, 1), (0, 1), (0, 1))]
 
 
-@pytest.mark.parametrize("n,bc", SHAPES[:5])
+@pytest.mark.parametrize("n,bc", SHAPES[:5] + SHAPES[7:])
 @pytest.mark.parametrize("opts", OPTS, ids=lambda d: "k%d-g%d-c%d" % (d["kernels"], d["graph"], d["coarse_cta"]))
 @pytest.mark.parametrize("nu", [(2, 2), (3, 3), (1, 0)])
 def test_vcycle_bit_exact(mgmod, uniform, n, bc, opts, nu):
