@@ -40,11 +40,29 @@ constexpr int SK_OY = 12;            // output rows per tile (rows 2..13)
 constexpr int SK_THREADS = SK_LX * SK_LY;
 
 struct SkSlot {                      // one z-plane of the tile in shared memory
-    double pe[SK_LY][SK_LX];         // p of even-x cells
-    double po[SK_LY][SK_LX];         // p of odd-x cells
-    double ae[SK_LY][SK_LX];         // a (level 0) of even-x cells
-    double ao[SK_LY][SK_LX];
+    double p[2][SK_LY][SK_LX];       // p by pair component (see "components" below)
+    double a[2][SK_LY][SK_LX];       // a = 0.5/rho (level 0 only)
 };
+
+constexpr int SK_DEPTH = 3;           // planes in flight beyond the one being collected
+constexpr int SK_NSTAGE = SK_DEPTH + 1;
+struct SkStage {                     // raw global layout of one plane of the tile (cp.async target)
+    double2 p[SK_LY][SK_LX];
+    double2 f[SK_LY][SK_LX];
+    double2 a[SK_LY][SK_LX];
+};
+constexpr size_t SK_SMEM_BYTES = 4 * sizeof(SkSlot) + SK_NSTAGE * sizeof(SkStage);
+
+__device__ __forceinline__ void sk_cp_async16(void *smem_dst, const void *gmem_src)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void sk_cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N> __device__ __forceinline__ void sk_cp_async_wait()
+{
+    asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
+}
 
 enum { SK_TAIL_NONE = 0, SK_TAIL_RESTRICT = 1, SK_TAIL_NORM = 2 };
 
@@ -53,7 +71,7 @@ struct SkArgs {
     const double *f;
     const double *pin;
     double *pout;
-    int zchunk;
+    int zchunk;                      // even
     // HEAD_PROLONG: coarse correction e (level+1) with its dims
     const double *e;
     int cnx, cny, cnz;
@@ -74,170 +92,228 @@ __device__ __forceinline__ int sk_map(int g, int n, int neumann, bool &ghost)
     if (m < 0 || m >= n) { m %= n; if (m < 0) m += n; }      // far ghost: value irrelevant
     return m;
 }
+// same for planes, which are never further than n away from the domain (no division)
+__device__ __forceinline__ int sk_map_near(int k, int n, int neumann, bool &ghost)
+{
+    ghost = false;
+    if (k < 0) { ghost = neumann; return neumann ? -1 - k : k + n; }
+    if (k >= n) { ghost = neumann; return neumann ? 2 * n - 1 - k : k - n; }
+    return k;
+}
 
+template <int V> struct SkInt { static constexpr int value = V; };
+
+// Components.  Thread (lx,ly) owns the cells (2lx, 2lx+1) of tile row ly, held as
+// component 0/1 such that component c has x-parity c ^ (ly & 1).  With the tile origin
+// even in x, y and the z-chunk origin even, the colour of component c at plane k is
+// (c + k) & 1 for EVERY thread: which component is red is a compile-time property of
+// the (6-fold unrolled) step, so the z-window lives in registers addressed by constants
+// (no rotation moves) and colour never costs a select.
 template <bool CELL, bool HEAD_PROLONG, int TAIL>
 __global__ void __launch_bounds__(SK_THREADS, 1) k_stream_sweep(SkArgs A)
 {
     extern __shared__ __align__(16) unsigned char sk_smem_raw[];
     SkSlot *slots = reinterpret_cast<SkSlot *>(sk_smem_raw);
+    SkStage *stages = reinterpret_cast<SkStage *>(sk_smem_raw + 4 * sizeof(SkSlot));
     const Lv &L = A.L;
     const int lx = threadIdx.x, ly = threadIdx.y;
+    const int rp = ly & 1;
     const int ox = blockIdx.x * SK_OX, oy = blockIdx.y * SK_OY;
     const int kz0 = blockIdx.z * A.zchunk;
     const int kz1 = min(L.nz, kz0 + A.zchunk);
+    const int so = ly * SK_LX + lx;              // offset inside one smem component plane
 
-    // ---- this thread's column: source indices of its pair and row
+    // ---- this thread's column
     const int gx = ox - 2 + 2 * lx;              // global x of the pair's even cell (may be outside)
     const int gy = oy - 2 + ly;
-    bool ghost_x0, ghost_x1, ghost_y;
-    const int sx0 = sk_map(gx, L.nx, L.bcx, ghost_x0);
-    const int sx1 = sk_map(gx + 1, L.nx, L.bcx, ghost_x1);
+    bool ghost_x, ghost_x1, ghost_y;
+    const int sx0 = sk_map(gx, L.nx, L.bcx, ghost_x);
+    const int sx1 = sk_map(gx + 1, L.nx, L.bcx, ghost_x1);   // ghost_x1 == ghost_x (nx even)
     const int sy = sk_map(gy, L.ny, L.bcy, ghost_y);
-    const bool swapx = sx1 < sx0;                 // mirrored pair: (sx1, sx0) is the aligned pair
-    const int sxp = swapx ? sx1 : sx0;            // aligned pair start (even)
-    const bool ghost_xy = ghost_x0 || ghost_y;    // ghost_x0 == ghost_x1 (pairs never straddle a wall)
-    const size_t col = (size_t)sxp + (size_t)L.nx * (size_t)sy;
+    const int xs0 = rp ? sx1 : sx0, xs1 = rp ? sx0 : sx1;    // source x of component 0 / 1
+    const size_t rowoff = (size_t)L.nx * (size_t)sy;
     const size_t plane_stride = (size_t)L.nx * L.ny;
-
+    const bool ghost_xy = ghost_x || ghost_y;
+    // x neighbour of component c lives in component c^1 of the thread at lx + dx(c)
+    const int dx0 = rp ? 1 : -1, dx1 = -dx0;
+    // smem offsets of the in-plane neighbours, clamped into the tile: edge threads read a
+    // valid (meaningless) word instead of branching; their results are never stored
+    const int so_x0 = min(max(so + dx0, 0), SK_LY * SK_LX - 1);
+    const int so_x1 = min(max(so + dx1, 0), SK_LY * SK_LX - 1);
+    const int so_ym = ly > 0 ? so - SK_LX : so;
+    const int so_yp = ly < SK_LY - 1 ? so + SK_LX : so;
     // region flags
-    const bool is_out = lx >= 1 && lx <= 30 && ly >= 2 && ly <= 13 && gx < L.nx && gy < L.ny &&
-                        gx >= 0 && gy >= 0;                   // owns output cells (both of the pair)
-    const bool row_r1 = ly >= 1 && ly <= 14 && !ghost_y;      // rows where red is (re)computed
+    const bool is_out = lx >= 1 && lx <= 30 && ly >= 2 && ly <= 13 && gx >= 0 && gx < L.nx &&
+                        gy >= 0 && gy < L.ny;
+    const bool row_r1 = ly >= 1 && ly <= 14 && !ghost_xy;
+    // component c sits at local x = 2lx + (c^rp); red is recomputed on local x in [1,62]
+    const bool red_ok0 = row_r1 && !(lx == 0 && rp == 0) && !(lx == 31 && rp == 1);
+    const bool red_ok1 = row_r1 && !(lx == 0 && rp == 1) && !(lx == 31 && rp == 0);
 
-    // register z-window: index 0 = plane t+1, 1 = t, 2 = t-1, 3 = t-2, 4 = t-3
-    double2 P[5], Aa[5], F[4];
+    // register z-window: ring of 6 planes; plane (t + d) of unrolled step U sits in (U+d) mod 6
+    double P[6][2], Aa[6][2], F[6][2];
 #pragma unroll
-    for (int q = 0; q < 5; ++q) { P[q] = make_double2(0.0, 0.0); Aa[q] = make_double2(0.0, 0.0); }
-#pragma unroll
-    for (int q = 0; q < 4; ++q) F[q] = make_double2(0.0, 0.0);
+    for (int q = 0; q < 6; ++q)
+        for (int c = 0; c < 2; ++c) { P[q][c] = 0.0; Aa[q][c] = 0.0; F[q][c] = 0.0; }
 
-    auto load_plane = [&](int k, double2 &p2, double2 &a2, double2 &f2) {
-        bool ghost_z;
-        const int sk = sk_map(k, L.nz, L.bcz, ghost_z);
-        const size_t idx = col + plane_stride * (size_t)sk;
-        p2 = *reinterpret_cast<const double2 *>(A.pin + idx);
-        f2 = *reinterpret_cast<const double2 *>(A.f + idx);
-        if (CELL) a2 = *reinterpret_cast<const double2 *>(L.a + idx);
-        if (swapx) {
-            double t_ = p2.x; p2.x = p2.y; p2.y = t_;
-            t_ = f2.x; f2.x = f2.y; f2.y = t_;
-            if (CELL) { t_ = a2.x; a2.x = a2.y; a2.y = t_; }
+    // aligned pair holding this thread's two cells, and which half is component 0
+    const int xpair = min(sx0, sx1);
+    const int c0_hi = xs0 > xs1 ? 1 : 0;          // component 0 is the odd-x (upper) word of the pair
+    // asynchronous copy of this thread's words of plane k into its staging buffer (LDGSTS:
+    // no registers are tied up, SK_DEPTH planes stay in flight per CTA)
+    auto issue = [&](int k) {
+        bool gz;
+        const int sk = sk_map_near(k, L.nz, L.bcz, gz);
+        const size_t idx = (size_t)xpair + rowoff + plane_stride * (size_t)sk;
+        SkStage &G = stages[k & (SK_NSTAGE - 1)];
+        sk_cp_async16(&G.p[ly][lx], A.pin + idx);
+        sk_cp_async16(&G.f[ly][lx], A.f + idx);
+        if (CELL) sk_cp_async16(&G.a[ly][lx], L.a + idx);
+        sk_cp_async_commit();
+    };
+    // pick the landed words of plane k out of the staging buffer into a ring entry
+    auto collect = [&](int k, double *p2, double *a2, double *f2, bool &ghost_z) {
+        const int sk = sk_map_near(k, L.nz, L.bcz, ghost_z);
+        const SkStage &G = stages[k & (SK_NSTAGE - 1)];
+        const double *gp = reinterpret_cast<const double *>(&G.p[ly][lx]);
+        const double *gf = reinterpret_cast<const double *>(&G.f[ly][lx]);
+        p2[0] = gp[c0_hi]; p2[1] = gp[c0_hi ^ 1];
+        f2[0] = gf[c0_hi]; f2[1] = gf[c0_hi ^ 1];
+        if (CELL) {
+            const double *ga = reinterpret_cast<const double *>(&G.a[ly][lx]);
+            a2[0] = ga[c0_hi]; a2[1] = ga[c0_hi ^ 1];
         }
-        if (CELL && (ghost_xy || ghost_z)) { a2.x = -a2.x; a2.y = -a2.y; }
         if (HEAD_PROLONG) {
-            // p_in + P e (C8) for both cells of the pair; ghosts keep the mirrored value,
-            // which is what the in-domain neighbour needs (it is multiplied by beta = 0)
-            p2.x = __dadd_rn(p2.x, prolong_value(L, A.e, A.cnx, A.cny, A.cnz, sx0, sy, sk));
-            p2.y = __dadd_rn(p2.y, prolong_value(L, A.e, A.cnx, A.cny, A.cnz, sx1, sy, sk));
+            p2[0] = __dadd_rn(p2[0], prolong_value(L, A.e, A.cnx, A.cny, A.cnz, xs0, sy, sk));
+            p2[1] = __dadd_rn(p2[1], prolong_value(L, A.e, A.cnx, A.cny, A.cnz, xs1, sy, sk));
         }
     };
-    auto store_slot = [&](int k, const double2 &p2, const double2 &a2) {
+    // finish a loaded plane: ghost sign of a, publish to the plane's smem slot
+    auto publish = [&](int k, double *p2, double *a2, bool ghost_z) {
         SkSlot &S = slots[k & 3];
-        S.pe[ly][lx] = p2.x; S.po[ly][lx] = p2.y;
-        if (CELL) { S.ae[ly][lx] = a2.x; S.ao[ly][lx] = a2.y; }
+        if (CELL) {
+            if (ghost_xy || ghost_z) { a2[0] = -a2[0]; a2[1] = -a2[1]; }
+            (&S.a[0][0][0])[so] = a2[0]; (&S.a[1][0][0])[so] = a2[1];
+        }
+        (&S.p[0][0][0])[so] = p2[0]; (&S.p[1][0][0])[so] = p2[1];
     };
 
-    // one Gauss-Seidel update (MODE 0) or residual (MODE 1) of cell `c` (0 = even-x cell,
-    // 1 = odd-x cell) of this thread's pair at the plane held in window index W (slot of
-    // plane k), using the window entries W-1 (plane k+1) and W+1 (plane k-1).
-    auto cell_SD = [&](int c, int k, int ks, const double2 &Pm, const double2 &Pc, const double2 &Pp,
-                       const double2 &Am, const double2 &Ac, const double2 &Ap, double &S_, double &D_) {
-        // Pm/Am: plane k-1, Pc/Ac: plane k, Pp/Ap: plane k+1
+    // S and D (C4) of component C of this thread's pair at plane k (smem slot k & 3; face
+    // arrays at wrapped plane ks); Pm/Pc/Pp = ring entries of planes k-1, k, k+1
+    auto cell_SD = [&](auto Cc, int k, int ks, const double *Pm, const double *Pc, const double *Pp,
+                       const double *Am, const double *Ac, const double *Ap, double &S_, double &D_) {
+        constexpr int C = decltype(Cc)::value;
         const SkSlot &S = slots[k & 3];
-        const double *own_p = c ? &S.po[0][0] : &S.pe[0][0];      // same x: y neighbours
-        const double *oth_p = c ? &S.pe[0][0] : &S.po[0][0];      // other parity: x neighbour
-        const int o = ly * SK_LX + lx;
-        const double p_partner = c ? Pc.x : Pc.y;
-        const double p_xnb = oth_p[o + (c ? 1 : -1)];
-        const double pxm = c ? p_partner : p_xnb;
-        const double pxp = c ? p_xnb : p_partner;
-        const double pym = own_p[o - SK_LX], pyp = own_p[o + SK_LX];
-        const double pzm = c ? Pm.y : Pm.x, pzp = c ? Pp.y : Pp.x;
+        const double *oth_p = &S.p[C ^ 1][0][0];
+        const bool left_is_smem = (C ? dx1 : dx0) < 0;
+        const double p_xnb = oth_p[C ? so_x1 : so_x0];
+        const double p_partner = Pc[C ^ 1];
+        const double pxm = left_is_smem ? p_xnb : p_partner;
+        const double pxp = left_is_smem ? p_partner : p_xnb;
+        const double pym = oth_p[so_ym], pyp = oth_p[so_yp];
+        const double pzm = Pm[C], pzp = Pp[C];
         double b[6];
         if (CELL) {
-            const double *own_a = c ? &S.ao[0][0] : &S.ae[0][0];
-            const double *oth_a = c ? &S.ae[0][0] : &S.ao[0][0];
-            const double a_c = c ? Ac.y : Ac.x;
-            const double a_partner = c ? Ac.x : Ac.y;
-            const double a_xnb = oth_a[o + (c ? 1 : -1)];
-            b[0] = __dadd_rn(a_c, c ? a_partner : a_xnb);
-            b[1] = __dadd_rn(a_c, c ? a_xnb : a_partner);
-            b[2] = __dadd_rn(a_c, own_a[o - SK_LX]);
-            b[3] = __dadd_rn(a_c, own_a[o + SK_LX]);
-            b[4] = __dadd_rn(a_c, c ? Am.y : Am.x);
-            b[5] = __dadd_rn(a_c, c ? Ap.y : Ap.x);
+            const double *oth_a = &S.a[C ^ 1][0][0];
+            const double a_c = Ac[C];
+            const double a_xnb = oth_a[C ? so_x1 : so_x0];
+            const double a_partner = Ac[C ^ 1];
+            b[0] = __dadd_rn(a_c, left_is_smem ? a_xnb : a_partner);
+            b[1] = __dadd_rn(a_c, left_is_smem ? a_partner : a_xnb);
+            b[2] = __dadd_rn(a_c, oth_a[so_ym]);
+            b[3] = __dadd_rn(a_c, oth_a[so_yp]);
+            b[4] = __dadd_rn(a_c, Am[C]);
+            b[5] = __dadd_rn(a_c, Ap[C]);
         } else {
             // stored minus faces, read through L1/L2 at the (wrapped) source position
-            const int x = c ? sx1 : sx0;
+            const int x = C ? xs1 : xs0;
             const int xp = x == L.nx - 1 ? 0 : x + 1;
             const int yp = sy == L.ny - 1 ? 0 : sy + 1;
             const int kp = ks == L.nz - 1 ? 0 : ks + 1;
-            const size_t cc = (size_t)x + (size_t)L.nx * ((size_t)sy + (size_t)L.ny * (size_t)ks);
+            const size_t pl = plane_stride * (size_t)ks;
+            const size_t cc = (size_t)x + rowoff + pl;
             b[0] = __ldg(L.bx + cc);
-            b[1] = __ldg(L.bx + ((size_t)xp + (size_t)L.nx * ((size_t)sy + (size_t)L.ny * (size_t)ks)));
+            b[1] = __ldg(L.bx + ((size_t)xp + rowoff + pl));
             b[2] = __ldg(L.by + cc);
-            b[3] = __ldg(L.by + ((size_t)x + (size_t)L.nx * ((size_t)yp + (size_t)L.ny * (size_t)ks)));
+            b[3] = __ldg(L.by + ((size_t)x + (size_t)L.nx * (size_t)yp + pl));
             b[4] = __ldg(L.bz + cc);
-            b[5] = __ldg(L.bz + ((size_t)x + (size_t)L.nx * ((size_t)sy + (size_t)L.ny * (size_t)kp)));
+            b[5] = __ldg(L.bz + ((size_t)x + rowoff + plane_stride * (size_t)kp));
         }
         S_ = stencil_S(b, pxm, pxp, pym, pyp, pzm, pzp);
         D_ = stencil_D(b);
     };
 
-    // ---- prologue: planes kz0-2, kz0-1, kz0 into window indices 2,1,0 of step t = kz0-1
+    const int t0 = kz0 - 1, t_end = kz1 + 1;
+    // ---- prologue: planes t0-1 .. t0+1 -> ring entries 5, 0, 1; SK_DEPTH more in flight
     {
-        double2 a2 = make_double2(0.0, 0.0);
-        load_plane(kz0 - 2, P[2], a2, F[2]); Aa[2] = a2; store_slot(kz0 - 2, P[2], Aa[2]);
-        load_plane(kz0 - 1, P[1], a2, F[1]); Aa[1] = a2; store_slot(kz0 - 1, P[1], Aa[1]);
-        load_plane(kz0,     P[0], a2, F[0]); Aa[0] = a2; store_slot(kz0,     P[0], Aa[0]);
+        static_assert(SK_NSTAGE == 4, "prologue stages exactly four planes");
+        issue(t0 - 1); issue(t0); issue(t0 + 1); issue(min(t0 + 2, kz1 + 1));
+        sk_cp_async_wait<1>();
+        bool gz;
+        collect(t0 - 1, P[5], Aa[5], F[5], gz); publish(t0 - 1, P[5], Aa[5], gz);
+        collect(t0,     P[0], Aa[0], F[0], gz); publish(t0,     P[0], Aa[0], gz);
+        collect(t0 + 1, P[1], Aa[1], F[1], gz); publish(t0 + 1, P[1], Aa[1], gz);
+        // their buffers are free again: bring the pipeline to SK_DEPTH planes in flight
+#pragma unroll
+        for (int d = 3; d <= 1 + SK_DEPTH; ++d) issue(min(t0 + d, kz1 + 1));
     }
     __syncthreads();
 
-    for (int t = kz0 - 1; t <= kz1 + 1; ++t) {
-        // prefetch plane t+2 (consumed at the end of this step)
-        double2 pn = make_double2(0.0, 0.0), an = make_double2(0.0, 0.0), fn = make_double2(0.0, 0.0);
-        const bool need_next = t + 2 <= kz1 + 1;
-        if (need_next) load_plane(t + 2, pn, an, fn);
+    // one step: red at plane t (ring U), black at plane t-2 (ring U+4), load plane t+2 (ring U+2)
+    auto step = [&](auto Uc, int t) {
+        constexpr int U = decltype(Uc)::value;
+        constexpr int R_P1 = (U + 1) % 6, R_0 = U % 6, R_M1 = (U + 5) % 6, R_M2 = (U + 4) % 6,
+                      R_M3 = (U + 3) % 6, R_P2 = (U + 2) % 6;
+        constexpr int RC = (1 + U) & 1;          // red component at plane t (t0 is odd)
+        constexpr int BC = RC ^ 1;               // black component at plane t-2
+        // keep SK_DEPTH planes in flight: plane t+2+SK_DEPTH goes into the staging buffer that
+        // plane t+1 left at the end of the previous step (always issued, clamped at the end)
+        issue(min(t + 2 + SK_DEPTH, kz1 + 1));
 
-        // -------- red half-sweep at plane t (window index 1)
-        {
-            const int cr = (oy + ly + t) & 1;          // which cell of the pair is red (x+y+z even)
-            bool ghost_z;
-            const int kt = sk_map(t, L.nz, L.bcz, ghost_z);
-            const int xl = 2 * lx + cr;                // local x of the red cell
-            const bool can = row_r1 && !ghost_x0 && !ghost_z && xl >= 1 && xl <= 62 && t <= kz1;
-            if (can) {
-                double S_, D_;
-                // the slot is keyed by the plane number t, the face arrays by the wrapped plane kt
-                cell_SD(cr, t, kt, P[2], P[1], P[0], Aa[2], Aa[1], Aa[0], S_, D_);
-                const double fv = cr ? F[1].y : F[1].x;
-                const double pv = gs_value(L.h2, fv, S_, D_);
-                if (cr) { P[1].y = pv; slots[t & 3].po[ly][lx] = pv; }
-                else    { P[1].x = pv; slots[t & 3].pe[ly][lx] = pv; }
-            }
+        // both updates are evaluated unconditionally (independent chains interleave);
+        // only the stores are predicated
+        bool ghost_z, ghost_zb;
+        const int kt = sk_map_near(t, L.nz, L.bcz, ghost_z);
+        const int kb = t - 2;
+        const int kbs = sk_map_near(kb, L.nz, L.bcz, ghost_zb);
+        double Sr, Dr, Sb, Db;
+        cell_SD(SkInt<RC>{}, t, kt, P[R_M1], P[R_0], P[R_P1], Aa[R_M1], Aa[R_0], Aa[R_P1], Sr, Dr);
+        cell_SD(SkInt<BC>{}, kb, kbs, P[R_M3], P[R_M2], P[R_M1], Aa[R_M3], Aa[R_M2], Aa[R_M1], Sb, Db);
+        const double pr = gs_value(L.h2, F[R_0][RC], Sr, Dr);
+        const double pb = gs_value(L.h2, F[R_M2][BC], Sb, Db);
+        // -------- red half-sweep at plane t
+        if ((RC ? red_ok1 : red_ok0) && !ghost_z && t <= kz1) {
+            P[R_0][RC] = pr;
+            (&slots[t & 3].p[RC][0][0])[so] = pr;
         }
-        // -------- black half-sweep at plane t-2 (window index 3)
-        {
-            const int kb = t - 2;
-            const int cb = ((oy + ly + t) & 1) ^ 1;
-            const bool can = is_out && kb >= kz0 && kb < kz1;
-            if (can) {
-                double S_, D_;
-                cell_SD(cb, kb, kb, P[4], P[3], P[2], Aa[4], Aa[3], Aa[2], S_, D_);
-                const double fv = cb ? F[3].y : F[3].x;
-                const double pv = gs_value(L.h2, fv, S_, D_);
-                if (cb) P[3].y = pv; else P[3].x = pv;
-                *reinterpret_cast<double2 *>(A.pout + col + plane_stride * (size_t)kb) = P[3];
-            }
+        // -------- black half-sweep at plane t-2
+        if (is_out && kb >= kz0 && kb < kz1) {
+            P[R_M2][BC] = pb;
+            double2 o2;
+            o2.x = rp ? P[R_M2][1] : P[R_M2][0];
+            o2.y = rp ? P[R_M2][0] : P[R_M2][1];
+            *reinterpret_cast<double2 *>(A.pout + (size_t)gx + rowoff + plane_stride * (size_t)kb) = o2;
         }
         __syncthreads();
-        // rotate the window and publish plane t+2
-#pragma unroll
-        for (int q = 4; q > 0; --q) { P[q] = P[q - 1]; Aa[q] = Aa[q - 1]; }
-#pragma unroll
-        for (int q = 3; q > 0; --q) F[q] = F[q - 1];
-        P[0] = pn; Aa[0] = an; F[0] = fn;
-        if (need_next) store_slot(t + 2, pn, an);
+        // plane t+2 has landed (all but the SK_DEPTH newest groups are complete)
+        sk_cp_async_wait<SK_DEPTH>();
+        bool gz_next;
+        collect(min(t + 2, kz1 + 1), P[R_P2], Aa[R_P2], F[R_P2], gz_next);
+        publish(t + 2, P[R_P2], Aa[R_P2], gz_next);
+    };
+
+    for (int tb = t0; tb <= t_end; tb += 6) {
+        step(SkInt<0>{}, tb);
+        if (tb + 1 > t_end) break;
+        step(SkInt<1>{}, tb + 1);
+        if (tb + 2 > t_end) break;
+        step(SkInt<2>{}, tb + 2);
+        if (tb + 3 > t_end) break;
+        step(SkInt<3>{}, tb + 3);
+        if (tb + 4 > t_end) break;
+        step(SkInt<4>{}, tb + 4);
+        if (tb + 5 > t_end) break;
+        step(SkInt<5>{}, tb + 5);
     }
 }
 
@@ -258,7 +334,7 @@ inline int sk_zchunk(int nx, int ny, int nz, int num_sms)
     if (zc < 16) zc = 16;
     if (zc > 64) zc = 64;
     if (zc > nz) zc = nz;
-    return zc;
+    return (zc + 1) & ~1;            // even: the colour of a component must not depend on the chunk
 }
 
 template <bool CELL>
@@ -266,7 +342,7 @@ inline int sk_launch_plain(const SkArgs &a, int num_sms, cudaStream_t st)
 {
     static bool attr_done = false;
     auto kern = k_stream_sweep<CELL, false, SK_TAIL_NONE>;
-    const size_t smem = 4 * sizeof(SkSlot);
+    const size_t smem = SK_SMEM_BYTES;
     if (!attr_done) {
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
             return -1;
