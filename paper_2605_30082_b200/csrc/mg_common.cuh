@@ -69,6 +69,12 @@ __device__ __forceinline__ double gs_value(double h2, double f, double S, double
 {
     return __dmul_rn(__fma_rn(-h2, f, S), __ddiv_rn(1.0, D));
 }
+// same value through the correctly rounded reciprocal instruction sequence: 1.0/D and
+// rcp(D) are both the round-to-nearest reciprocal, hence identical bits
+__device__ __forceinline__ double gs_value_rcp(double h2, double f, double S, double D)
+{
+    return __dmul_rn(__fma_rn(-h2, f, S), __drcp_rn(D));
+}
 __device__ __forceinline__ double resid_value(double ih2, double f, double S, double D, double p)
 {
     return __fma_rn(-ih2, __fma_rn(-D, p, S), f);

@@ -53,9 +53,8 @@ struct SkStage {                     // raw global layout of one plane of the ti
 };
 constexpr size_t SK_SMEM_BYTES = 4 * sizeof(SkSlot) + SK_NSTAGE * sizeof(SkStage);
 
-__device__ __forceinline__ void sk_cp_async16(void *smem_dst, const void *gmem_src)
+__device__ __forceinline__ void sk_cp_async16(unsigned d, const void *gmem_src)
 {
-    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src) : "memory");
 }
 __device__ __forceinline__ void sk_cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
@@ -109,15 +108,14 @@ template <int V> struct SkInt { static constexpr int value = V; };
 // (c + k) & 1 for EVERY thread: which component is red is a compile-time property of
 // the (6-fold unrolled) step, so the z-window lives in registers addressed by constants
 // (no rotation moves) and colour never costs a select.
-template <bool CELL, bool HEAD_PROLONG, int TAIL>
-__global__ void __launch_bounds__(SK_THREADS, 1) k_stream_sweep(SkArgs A)
+template <bool CELL, bool HEAD_PROLONG, int TAIL, int RP>
+__device__ __forceinline__ void sk_body(const SkArgs &A, unsigned char *sk_smem_raw)
 {
-    extern __shared__ __align__(16) unsigned char sk_smem_raw[];
     SkSlot *slots = reinterpret_cast<SkSlot *>(sk_smem_raw);
     SkStage *stages = reinterpret_cast<SkStage *>(sk_smem_raw + 4 * sizeof(SkSlot));
     const Lv &L = A.L;
     const int lx = threadIdx.x, ly = threadIdx.y;
-    const int rp = ly & 1;
+    constexpr int rp = RP;                       // row parity = ly & 1 (warp-uniform)
     const int ox = blockIdx.x * SK_OX, oy = blockIdx.y * SK_OY;
     const int kz0 = blockIdx.z * A.zchunk;
     const int kz1 = min(L.nz, kz0 + A.zchunk);
@@ -135,7 +133,7 @@ __global__ void __launch_bounds__(SK_THREADS, 1) k_stream_sweep(SkArgs A)
     const size_t plane_stride = (size_t)L.nx * L.ny;
     const bool ghost_xy = ghost_x || ghost_y;
     // x neighbour of component c lives in component c^1 of the thread at lx + dx(c)
-    const int dx0 = rp ? 1 : -1, dx1 = -dx0;
+    constexpr int dx0 = rp ? 1 : -1, dx1 = -dx0;
     // smem offsets of the in-plane neighbours, clamped into the tile: edge threads read a
     // valid (meaningless) word instead of branching; their results are never stored
     const int so_x0 = min(max(so + dx0, 0), SK_LY * SK_LX - 1);
@@ -156,19 +154,26 @@ __global__ void __launch_bounds__(SK_THREADS, 1) k_stream_sweep(SkArgs A)
     for (int q = 0; q < 6; ++q)
         for (int c = 0; c < 2; ++c) { P[q][c] = 0.0; Aa[q][c] = 0.0; F[q][c] = 0.0; }
 
+    const unsigned stage_addr = (unsigned)__cvta_generic_to_shared(&stages[0].p[ly][lx]);
     // aligned pair holding this thread's two cells, and which half is component 0
     const int xpair = min(sx0, sx1);
     const int c0_hi = xs0 > xs1 ? 1 : 0;          // component 0 is the odd-x (upper) word of the pair
     // asynchronous copy of this thread's words of plane k into its staging buffer (LDGSTS:
     // no registers are tied up, SK_DEPTH planes stay in flight per CTA)
+    // per-thread base pointers of the three streams; a plane is one 32x32->64 bit
+    // multiply-add away (plane stride in bytes < 2^32, checked on the host)
+    const unsigned plane_bytes = (unsigned)(plane_stride * sizeof(double));
+    const char *src_p = reinterpret_cast<const char *>(A.pin + (size_t)xpair + rowoff);
+    const char *src_f = reinterpret_cast<const char *>(A.f + (size_t)xpair + rowoff);
+    const char *src_a = CELL ? reinterpret_cast<const char *>(L.a + (size_t)xpair + rowoff) : nullptr;
     auto issue = [&](int k) {
         bool gz;
-        const int sk = sk_map_near(k, L.nz, L.bcz, gz);
-        const size_t idx = (size_t)xpair + rowoff + plane_stride * (size_t)sk;
-        SkStage &G = stages[k & (SK_NSTAGE - 1)];
-        sk_cp_async16(&G.p[ly][lx], A.pin + idx);
-        sk_cp_async16(&G.f[ly][lx], A.f + idx);
-        if (CELL) sk_cp_async16(&G.a[ly][lx], L.a + idx);
+        const unsigned sk = (unsigned)sk_map_near(k, L.nz, L.bcz, gz);
+        const size_t off = (size_t)sk * plane_bytes;
+        const unsigned g = stage_addr + (unsigned)(k & (SK_NSTAGE - 1)) * (unsigned)sizeof(SkStage);
+        sk_cp_async16(g, src_p + off);
+        sk_cp_async16(g + (unsigned)sizeof(double2) * SK_LY * SK_LX, src_f + off);
+        if (CELL) sk_cp_async16(g + 2u * (unsigned)sizeof(double2) * SK_LY * SK_LX, src_a + off);
         sk_cp_async_commit();
     };
     // pick the landed words of plane k out of the staging buffer into a ring entry
@@ -205,7 +210,7 @@ __global__ void __launch_bounds__(SK_THREADS, 1) k_stream_sweep(SkArgs A)
         constexpr int C = decltype(Cc)::value;
         const SkSlot &S = slots[k & 3];
         const double *oth_p = &S.p[C ^ 1][0][0];
-        const bool left_is_smem = (C ? dx1 : dx0) < 0;
+        constexpr bool left_is_smem = (C ? dx1 : dx0) < 0;
         const double p_xnb = oth_p[C ? so_x1 : so_x0];
         const double p_partner = Pc[C ^ 1];
         const double pxm = left_is_smem ? p_xnb : p_partner;
@@ -279,8 +284,8 @@ __global__ void __launch_bounds__(SK_THREADS, 1) k_stream_sweep(SkArgs A)
         double Sr, Dr, Sb, Db;
         cell_SD(SkInt<RC>{}, t, kt, P[R_M1], P[R_0], P[R_P1], Aa[R_M1], Aa[R_0], Aa[R_P1], Sr, Dr);
         cell_SD(SkInt<BC>{}, kb, kbs, P[R_M3], P[R_M2], P[R_M1], Aa[R_M3], Aa[R_M2], Aa[R_M1], Sb, Db);
-        const double pr = gs_value(L.h2, F[R_0][RC], Sr, Dr);
-        const double pb = gs_value(L.h2, F[R_M2][BC], Sb, Db);
+        const double pr = gs_value_rcp(L.h2, F[R_0][RC], Sr, Dr);
+        const double pb = gs_value_rcp(L.h2, F[R_M2][BC], Sb, Db);
         // -------- red half-sweep at plane t
         if ((RC ? red_ok1 : red_ok0) && !ghost_z && t <= kz1) {
             P[R_0][RC] = pr;
@@ -317,12 +322,21 @@ __global__ void __launch_bounds__(SK_THREADS, 1) k_stream_sweep(SkArgs A)
     }
 }
 
+template <bool CELL, bool HEAD_PROLONG, int TAIL>
+__global__ void __launch_bounds__(SK_THREADS, 1) k_stream_sweep(SkArgs A)
+{
+    extern __shared__ __align__(16) unsigned char sk_smem_raw[];
+    // a warp is one tile row, so the row parity is warp-uniform: two specialised bodies
+    if (threadIdx.y & 1) sk_body<CELL, HEAD_PROLONG, TAIL, 1>(A, sk_smem_raw);
+    else                 sk_body<CELL, HEAD_PROLONG, TAIL, 0>(A, sk_smem_raw);
+}
+
 // ------------------------------------------------------------------------------ host side
 inline bool stream_sweep_supported(int nx, int ny, int nz)
 {
     // any even dims work; below 32^3 the launch is latency-bound and the reference /
     // single-CTA kernels are used instead
-    return nx >= 32 && ny >= 32 && nz >= 32;
+    return nx >= 32 && ny >= 32 && nz >= 32 && (size_t)nx * ny * sizeof(double) < 0xffffffffull;
 }
 
 inline int sk_zchunk(int nx, int ny, int nz, int num_sms)
