@@ -23,7 +23,7 @@ NVCC_FLAGS = [
     "-lineinfo", "-O3", "-std=c++17",
     "-fmad=false",                 # no implicit contraction: all fma are explicit
     "-Xcompiler", "-fPIC", "-shared",
-]
+] + os.environ.get("MG_NVCC_EXTRA", "").split()     # e.g. -DS3_BAR2=0 for kernel experiments
 
 
 def sources():
