@@ -44,7 +44,10 @@ constexpr int S3_NSLOT = 6;
 #define S3_BAR2 1
 #endif
 constexpr int S3_FPF = 4;                 // L2 prefetch distance of the f stream (planes beyond t+1)
-constexpr int S3_NST = 3;                 // staging planes in flight (cp.async)
+#ifndef S3_NST_
+#define S3_NST_ 3
+#endif
+constexpr int S3_NST = S3_NST_;                 // staging planes in flight (cp.async)
 
 constexpr int S3_COMP_BYTES = S3_TY * S3_LX * 16;        // one colour class of one plane
 constexpr int S3_SLOT_BYTES = 2 * S3_COMP_BYTES;
@@ -169,7 +172,8 @@ __device__ __forceinline__ void s3_body(const S3Args &A, unsigned smem_base)
     // ---- region predicates
     const bool is_out = lx >= 1 && lx <= S3_LX - 2 && ly >= 2 && ly <= S3_TY - 3 && gx >= 0 && gx < L.nx &&
                         gy >= 0 && gy < L.ny;
-    const bool row_r1 = ly >= 1 && ly <= S3_TY - 2 && !ghost_xy;
+    const bool w_work = ly >= 1 && ly <= S3_TY - 2;       // warp-uniform: rows that compute at all
+    const bool row_r1 = w_work && !ghost_xy;
     // red is recomputed on local x in [1, 62]: everything but the outermost cell of the edge lanes
     const bool red_ok_lo = row_r1 && lx != 0;               // cell at local x = 2lx
     const bool red_ok_hi = row_r1 && lx != S3_LX - 1;       // cell at local x = 2lx + 1
@@ -203,7 +207,7 @@ __device__ __forceinline__ void s3_body(const S3Args &A, unsigned smem_base)
     // step; the store of plane t-2 is seven planes behind it (is_out threads load and store
     // the same pair)
     size_t roff = col_bytes;
-    const size_t back7 = 7 * plane_bytes;
+    const size_t back_store = (size_t)(S3_NST + 4) * plane_bytes, back_f = (size_t)S3_NST * plane_bytes;
     // move a landed plane from staging slot SLOT into ring entry R and publish it to exchange slot R
     auto take = [&](auto Rc, auto Sc, unsigned sign) __attribute__((always_inline)) {
         constexpr int R = decltype(Rc)::value;
@@ -279,13 +283,22 @@ __device__ __forceinline__ void s3_body(const S3Args &A, unsigned smem_base)
 
     const int t0 = kz0 - 1, t_end = kz1 + 1;
     // ---- prologue: planes t0-1, t0, t0+1 -> ring entries 5, 0, 1; plane t0+2 in flight
-    issue(S3Int<2>{}, t0 - 1); issue(S3Int<0>{}, t0); issue(S3Int<1>{}, t0 + 1);
-    if (S3_FDIRECT) load_f(S3Int<0>{}, zoff(t0));
+    // (plane k uses staging slot (k - t0) mod S3_NST)
+    static_assert(S3_NST == 3 || S3_NST == 6, "staging depth must divide the unroll factor");
+    issue(S3Int<S3_NST - 1>{}, t0 - 1); issue(S3Int<0>{}, t0); issue(S3Int<1>{}, t0 + 1);
+    if (S3_FDIRECT) { load_f(S3Int<0>{}, zoff(t0)); load_f(S3Int<1>{}, zoff(t0 + 1)); }
     s3_cp_async_wait<0>();
-    take(S3Int<5>{}, S3Int<2>{}, zsign(t0 - 1));
+    take(S3Int<5>{}, S3Int<S3_NST - 1>{}, zsign(t0 - 1));
     take(S3Int<0>{}, S3Int<0>{}, zsign(t0));
     take(S3Int<1>{}, S3Int<1>{}, zsign(t0 + 1));
-    issue(S3Int<2>{}, min(t0 + 2, kz1 + 1)); issue(S3Int<0>{}, min(t0 + 3, kz1 + 1)); issue(S3Int<1>{}, min(t0 + 4, kz1 + 1));
+    issue(S3Int<2 % S3_NST>{}, min(t0 + 2, kz1 + 1));
+    issue(S3Int<3 % S3_NST>{}, min(t0 + 3, kz1 + 1));
+    issue(S3Int<4 % S3_NST>{}, min(t0 + 4, kz1 + 1));
+    if (S3_NST == 6) {
+        issue(S3Int<5 % S3_NST>{}, min(t0 + 5, kz1 + 1));
+        issue(S3Int<6 % S3_NST>{}, min(t0 + 6, kz1 + 1));
+        issue(S3Int<7 % S3_NST>{}, min(t0 + 7, kz1 + 1));
+    }
     __syncthreads();
 
     // one step: red at plane t (ring U), black at plane t-2 (ring U+4), plane t+2 enters ring
@@ -301,16 +314,18 @@ __device__ __forceinline__ void s3_body(const S3Args &A, unsigned smem_base)
         const int kb = t - 2;
         const int kt = STEADY ? t : s3_zmap(t, L.nz, L.bcz, sg_t);
         const int kbs = STEADY ? kb : s3_zmap(kb, L.nz, L.bcz, sg_b);
-        // f of plane t+1 -> ring (first used by the next step)
+        // f of plane t+2 -> ring (first used two steps later)
         if (!S3_FDIRECT) {
         } else if (STEADY) {
-            load_f(S3Int<(U + 1) % 6>{}, roff - 4 * plane_bytes);
-            s3_prefetch_l2(base_f + roff + (S3_FPF - 4) * plane_bytes);
+            load_f(S3Int<(U + 2) % 6>{}, roff - back_f);
+            s3_prefetch_l2(base_f + (roff - back_f) + S3_FPF * plane_bytes);
         } else {
-            load_f(S3Int<(U + 1) % 6>{}, zoff(min(t + 1, kz1 + 1)));
+            load_f(S3Int<(U + 2) % 6>{}, zoff(min(t + 2, kz1 + 1)));
         }
-        // both updates are evaluated unconditionally (two independent chains interleave);
-        // only the stores are predicated
+        // Ring-2 rows (the first and the last warp) only move data.  Everywhere else both
+        // updates are evaluated unconditionally (two independent chains interleave); only
+        // the stores are predicated.
+        if (w_work) {
         const double pr = gs(S3Int<RC>{}, S3Int<R_0>{}, kt);
         const double pb = gs(S3Int<BC>{}, S3Int<R_M2>{}, kbs);
         // -------- red half-sweep at plane t
@@ -324,17 +339,18 @@ __device__ __forceinline__ void s3_body(const S3Args &A, unsigned smem_base)
             double2 o2;
             o2.x = P[R_M2][C_LO];
             o2.y = P[R_M2][C_HI];
-            if (STEADY) *reinterpret_cast<double2 *>(reinterpret_cast<char *>(A.pout) + (roff - back7)) = o2;
+            if (STEADY) *reinterpret_cast<double2 *>(reinterpret_cast<char *>(A.pout) + (roff - back_store)) = o2;
             else *reinterpret_cast<double2 *>(A.pout + (size_t)gx + (size_t)L.nx * (size_t)gy +
                                               plane_stride * (size_t)kb) = o2;
         }
+        }
         // -------- plane t+2 (in flight for three steps) enters the ring and its exchange
         // slot (last read two barriers ago); plane t+5 goes in flight into the freed staging slot
-        constexpr int SLOT = (U + 2) % 3;
+        constexpr int SLOT = (U + 2) % S3_NST;
         s3_cp_async_wait<S3_NST - 1>();
         take(S3Int<R_P2>{}, S3Int<SLOT>{}, STEADY ? sign_xy : zsign(min(t + 2, kz1 + 1)));
         if (STEADY) { issue_at(S3Int<SLOT>{}, roff); roff += plane_bytes; }
-        else issue(S3Int<SLOT>{}, min(t + 5, kz1 + 1));
+        else issue(S3Int<SLOT>{}, min(t + 2 + S3_NST, kz1 + 1));
         // Shared-memory writes of step t (red values of plane t, publication of plane t+2) are
         // first read in step t+2, and the exchange slot written in step t was last read in step
         // t-2: one barrier every second step orders both.
@@ -355,10 +371,10 @@ __device__ __forceinline__ void s3_body(const S3Args &A, unsigned smem_base)
 
     int t = t0;
     // steady steps: t in [kz0+2, ts_end]; entered at ring position 3 (t0 + 3 = kz0 + 2)
-    const int ts_end = min(kz1 - 4, L.nz - 6);
+    const int ts_end = min(kz1 - 1 - S3_NST, L.nz - 3 - S3_NST);
     generic_steps(t, min(kz0 + 1, t_end));
     if (t + 5 <= ts_end) {
-        roff = col_bytes + (size_t)(t + 5) * plane_bytes;
+        roff = col_bytes + (size_t)(t + 2 + S3_NST) * plane_bytes;
         for (; t + 5 <= ts_end; t += 6) {
             step(S3Int<3>{}, S3Int<1>{}, t);
             step(S3Int<4>{}, S3Int<1>{}, t + 1);

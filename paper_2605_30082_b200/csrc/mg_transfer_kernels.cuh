@@ -1,0 +1,272 @@
+// mg_transfer_kernels.cuh -- streaming kernels for the residual-based steps of the cycle:
+//   k_resid_stream<CELL, RS_RESTRICT> : A2+A3, r = f - A p on the fly, 8-child mean written to
+//                                       the coarse right-hand side (r never materialised)
+//   k_resid_stream<CELL, RS_NORM>     : A7, sum of r^2 per block (deterministic tree)
+//   k_prolong_stream                  : A5, p_out = p_in + P e (out of place or in place)
+//
+// Geometry of k_resid_stream.  A warp owns a ROW PAIR (rows 2J, 2J+1) of a 64-cell wide
+// strip and marches along z; lane lx owns the aligned x-pairs (2lx, 2lx+1) of both rows,
+// i.e. the 2x2 in-plane footprint of one coarse cell, and keeps the z-window (planes k-1,
+// k, k+1) of its four cells of p and a in registers.  Every global access is a coalesced
+// 16-byte load; the x-neighbours come from the adjacent lanes by warp shuffle (the two
+// edge lanes load one scalar), the y-neighbours of the row pair are two more row loads
+// (L1/L2 hits: they are the own rows of the warps above and below).  Compulsory traffic:
+// 24 B per cell (p, f, a) + 1 B (coarse rhs).
+//
+// Boundaries as in the sweep kernel: a periodic neighbour is the wrapped index; across a
+// Neumann wall the neighbour coefficient is taken as -a_c, so that the face a_c + a_nb is
+// exactly +0.0 (C2), and the neighbour value is the (finite) mirror cell.  Coarse levels
+// read their stored minus-face arrays (which hold 0 on a wall).
+#pragma once
+#include "mg_common.cuh"
+
+namespace mg {
+
+constexpr int RS_WARPS = 4;               // row pairs per block
+constexpr int RS_THREADS = 32 * RS_WARPS;
+enum { RS_NORM = 0, RS_RESTRICT = 1 };
+
+struct RsArgs {
+    Lv L;
+    const double *f;
+    const double *p;
+    double *fc;            // RS_RESTRICT: coarse rhs (cnx x cny x nz/2)
+    int cnx, cny;
+    double *partial;       // RS_NORM: one partial sum per block
+    int zchunk;            // even
+};
+
+__device__ __forceinline__ double2 rs_ld2(const double *base, size_t idx)
+{
+    return __ldg(reinterpret_cast<const double2 *>(base + idx));
+}
+__device__ __forceinline__ double2 rs_neg(double2 v) { return make_double2(-v.x, -v.y); }
+
+// residual (C4, C6) of one cell from its six faces and neighbour values
+__device__ __forceinline__ double rs_resid(const double b[6], double pxm, double pxp, double pym,
+                                           double pyp, double pzm, double pzp, double pc, double f,
+                                           double ih2)
+{
+    const double S = stencil_S(b, pxm, pxp, pym, pyp, pzm, pzp);
+    const double D = stencil_D(b);
+    return resid_value(ih2, f, S, D, pc);
+}
+
+template <bool CELL, int MODE>
+__global__ void __launch_bounds__(RS_THREADS) k_resid_stream(RsArgs A)
+{
+    const Lv &L = A.L;
+    const int lx = threadIdx.x;
+    const int x0r = (blockIdx.x * 32 + lx) * 2;                     // even x of the pair (may be >= nx)
+    const int Jr = blockIdx.y * RS_WARPS + threadIdx.y;             // row pair (may be outside)
+    const bool valid = x0r < L.nx && 2 * Jr < L.ny;
+    const int x0 = min(x0r, L.nx - 2), j0 = min(2 * Jr, L.ny - 2), j1 = j0 + 1;
+    const int kz0 = blockIdx.z * A.zchunk, kz1 = min(L.nz, kz0 + A.zchunk);
+
+    // in-plane neighbour indices (always the wrapped index: across a Neumann wall the face is
+    // forced to +0.0, so any finite neighbour value does) and wall flags
+    const bool wall_xl = L.bcx && x0 == 0, wall_xr = L.bcx && x0 + 2 == L.nx;
+    const bool wall_y0 = L.bcy && j0 == 0, wall_y1 = L.bcy && j1 == L.ny - 1;
+    const int xl = x0 == 0 ? L.nx - 1 : x0 - 1;                     // left neighbour of the even cell
+    const int xr = x0 + 2 == L.nx ? 0 : x0 + 2;                     // right neighbour of the odd cell
+    const int jm = j0 == 0 ? L.ny - 1 : j0 - 1;
+    const int jp = j1 == L.ny - 1 ? 0 : j1 + 1;
+    const bool edge_l = lx == 0, edge_r = lx == 31 || x0 + 2 >= L.nx;
+    const size_t plane = (size_t)L.nx * L.ny;
+    const size_t row0 = (size_t)L.nx * j0, row1 = (size_t)L.nx * j1, rowm = (size_t)L.nx * jm, rowp = (size_t)L.nx * jp;
+
+    // z-window of the own rows: [r] = row j0 / j1
+    double2 Pm[2], Pc[2], Pp[2], Am[2], Ac[2], Ap[2], Bzc[2], Bzp[2];
+    auto zprev = [&](int k) { return k == 0 ? L.nz - 1 : k - 1; };
+    auto znext = [&](int k) { return k == L.nz - 1 ? 0 : k + 1; };
+    {
+        const size_t om = plane * (size_t)zprev(kz0), oc = plane * (size_t)kz0;
+        Pm[0] = rs_ld2(A.p, om + row0 + x0); Pm[1] = rs_ld2(A.p, om + row1 + x0);
+        Pc[0] = rs_ld2(A.p, oc + row0 + x0); Pc[1] = rs_ld2(A.p, oc + row1 + x0);
+        if (CELL) {
+            Am[0] = rs_ld2(L.a, om + row0 + x0); Am[1] = rs_ld2(L.a, om + row1 + x0);
+            Ac[0] = rs_ld2(L.a, oc + row0 + x0); Ac[1] = rs_ld2(L.a, oc + row1 + x0);
+        } else {
+            Bzc[0] = rs_ld2(L.bz, oc + row0 + x0); Bzc[1] = rs_ld2(L.bz, oc + row1 + x0);
+        }
+    }
+    double acc = 0.0;          // RS_NORM: running sum of r^2; RS_RESTRICT: plane sum of the even plane
+
+    for (int k = kz0; k < kz1; ++k) {
+        const size_t oc = plane * (size_t)k, op = plane * (size_t)znext(k);
+        const bool wall_z0 = L.bcz && k == 0, wall_z1 = L.bcz && k == L.nz - 1;
+        // ---- loads of this plane: next plane of the own rows, the two neighbour rows, f
+        Pp[0] = rs_ld2(A.p, op + row0 + x0); Pp[1] = rs_ld2(A.p, op + row1 + x0);
+        const double2 Pym = rs_ld2(A.p, oc + rowm + x0), Pyp = rs_ld2(A.p, oc + rowp + x0);
+        const double2 F0 = rs_ld2(A.f, oc + row0 + x0), F1 = rs_ld2(A.f, oc + row1 + x0);
+        double2 Aym, Ayp, Bx[2], By[3];
+        if (CELL) {
+            Ap[0] = rs_ld2(L.a, op + row0 + x0); Ap[1] = rs_ld2(L.a, op + row1 + x0);
+            Aym = rs_ld2(L.a, oc + rowm + x0); Ayp = rs_ld2(L.a, oc + rowp + x0);
+        } else {
+            Bzp[0] = rs_ld2(L.bz, op + row0 + x0); Bzp[1] = rs_ld2(L.bz, op + row1 + x0);
+            Bx[0] = rs_ld2(L.bx, oc + row0 + x0); Bx[1] = rs_ld2(L.bx, oc + row1 + x0);
+            By[0] = rs_ld2(L.by, oc + row0 + x0); By[1] = rs_ld2(L.by, oc + row1 + x0);
+            By[2] = rs_ld2(L.by, oc + rowp + x0);
+        }
+        // ---- x-neighbours: adjacent lanes; the two edge lanes load a scalar
+        double pl[2], pr[2], al[2], ar[2], bxr[2];
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            const size_t row = r ? row1 : row0;
+            pl[r] = __shfl_up_sync(0xffffffffu, Pc[r].y, 1);
+            pr[r] = __shfl_down_sync(0xffffffffu, Pc[r].x, 1);
+            if (edge_l) pl[r] = __ldg(A.p + oc + row + xl);
+            if (edge_r) pr[r] = __ldg(A.p + oc + row + xr);
+            if (CELL) {
+                al[r] = __shfl_up_sync(0xffffffffu, Ac[r].y, 1);
+                ar[r] = __shfl_down_sync(0xffffffffu, Ac[r].x, 1);
+                if (edge_l) al[r] = __ldg(L.a + oc + row + xl);
+                if (edge_r) ar[r] = __ldg(L.a + oc + row + xr);
+                if (wall_xl) al[r] = -Ac[r].x;
+                if (wall_xr) ar[r] = -Ac[r].y;
+            } else {
+                bxr[r] = __shfl_down_sync(0xffffffffu, Bx[r].x, 1);
+                if (edge_r) bxr[r] = __ldg(L.bx + oc + row + xr);
+            }
+        }
+        // ---- residuals of the 2x2 footprint: res[r][xi]
+        double res[2][2];
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+#pragma unroll
+            for (int xi = 0; xi < 2; ++xi) {
+                const double pc = xi ? Pc[r].y : Pc[r].x;
+                const double pxm = xi ? Pc[r].x : pl[r];
+                const double pxp = xi ? pr[r] : Pc[r].y;
+                const double pym = r ? (xi ? Pc[0].y : Pc[0].x) : (xi ? Pym.y : Pym.x);
+                const double pyp = r ? (xi ? Pyp.y : Pyp.x) : (xi ? Pc[1].y : Pc[1].x);
+                const double pzm = xi ? Pm[r].y : Pm[r].x;
+                const double pzp = xi ? Pp[r].y : Pp[r].x;
+                const double fv = r ? (xi ? F1.y : F1.x) : (xi ? F0.y : F0.x);
+                double b[6];
+                if (CELL) {
+                    const double a_c = xi ? Ac[r].y : Ac[r].x;
+                    const double axm = xi ? Ac[r].x : al[r];
+                    const double axp = xi ? ar[r] : Ac[r].y;
+                    double aym = r ? (xi ? Ac[0].y : Ac[0].x) : (xi ? Aym.y : Aym.x);
+                    double ayp = r ? (xi ? Ayp.y : Ayp.x) : (xi ? Ac[1].y : Ac[1].x);
+                    double azm = xi ? Am[r].y : Am[r].x;
+                    double azp = xi ? Ap[r].y : Ap[r].x;
+                    if (r == 0 && wall_y0) aym = -a_c;
+                    if (r == 1 && wall_y1) ayp = -a_c;
+                    if (wall_z0) azm = -a_c;
+                    if (wall_z1) azp = -a_c;
+                    b[0] = __dadd_rn(a_c, axm); b[1] = __dadd_rn(a_c, axp);
+                    b[2] = __dadd_rn(a_c, aym); b[3] = __dadd_rn(a_c, ayp);
+                    b[4] = __dadd_rn(a_c, azm); b[5] = __dadd_rn(a_c, azp);
+                } else {
+                    b[0] = xi ? Bx[r].y : Bx[r].x;
+                    b[1] = xi ? bxr[r] : Bx[r].y;
+                    b[2] = xi ? By[r].y : By[r].x;
+                    b[3] = xi ? By[r + 1].y : By[r + 1].x;
+                    b[4] = xi ? Bzc[r].y : Bzc[r].x;
+                    b[5] = xi ? Bzp[r].y : Bzp[r].x;
+                }
+                res[r][xi] = rs_resid(b, pxm, pxp, pym, pyp, pzm, pzp, pc, fv, L.ih2);
+            }
+        }
+        if (MODE == RS_RESTRICT) {
+            // C7: ((r000+r100)+(r010+r110)) + ((r001+r101)+(r011+r111)), index order x,y,z
+            const double ps = __dadd_rn(__dadd_rn(res[0][0], res[0][1]), __dadd_rn(res[1][0], res[1][1]));
+            if (k & 1) {
+                if (valid)
+                    A.fc[(size_t)(x0 >> 1) + (size_t)A.cnx * ((size_t)(j0 >> 1) + (size_t)A.cny * (size_t)(k >> 1))] =
+                        __dmul_rn(0.125, __dadd_rn(acc, ps));
+            } else {
+                acc = ps;
+            }
+        } else if (valid) {
+            acc = __fma_rn(res[0][0], res[0][0], acc);
+            acc = __fma_rn(res[0][1], res[0][1], acc);
+            acc = __fma_rn(res[1][0], res[1][0], acc);
+            acc = __fma_rn(res[1][1], res[1][1], acc);
+        }
+        // ---- rotate the window
+        Pm[0] = Pc[0]; Pm[1] = Pc[1]; Pc[0] = Pp[0]; Pc[1] = Pp[1];
+        if (CELL) { Am[0] = Ac[0]; Am[1] = Ac[1]; Ac[0] = Ap[0]; Ac[1] = Ap[1]; }
+        else { Bzc[0] = Bzp[0]; Bzc[1] = Bzp[1]; }
+    }
+    if (MODE == RS_NORM) {
+        __shared__ double red[32];
+        acc = block_sum(acc, red);
+        if (threadIdx.x == 0 && threadIdx.y == 0)
+            A.partial[blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z)] = acc;
+    }
+}
+
+// ---- A5: p_out = p_in + P e (C8), one thread per COARSE cell = 2x2x2 fine cells -----------
+// The 27 coarse values around (I,J,K) are read once (coalesced along I, L1/L2 hits for the
+// overlap) and the tensor-product interpolation shares its x- and y-stages between the 8
+// children: 38 lerps instead of 56.  Fine data moves as 16-byte pairs.  p_out may be p_in.
+struct PrArgs {
+    int nx, ny, nz;            // fine dims
+    int cnx, cny, cnz;         // coarse dims
+    int bcx, bcy, bcz;
+    const double *e;
+    const double *pin;
+    double *pout;
+};
+
+__device__ __forceinline__ int pr_nb(int I, int d, int n, int neumann)
+{
+    int q = I + d;
+    if (q < 0) q = neumann ? 0 : n - 1;
+    if (q >= n) q = neumann ? n - 1 : 0;
+    return q;
+}
+
+__global__ void __launch_bounds__(128) k_prolong_stream(PrArgs A)
+{
+    const int I = blockIdx.x * 32 + threadIdx.x;
+    const int J = blockIdx.y * 4 + threadIdx.y;
+    const int K = blockIdx.z;
+    if (I >= A.cnx || J >= A.cny) return;
+    int xi[3], yj[3], zk[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        xi[d] = pr_nb(I, d - 1, A.cnx, A.bcx);
+        yj[d] = pr_nb(J, d - 1, A.cny, A.bcy);
+        zk[d] = pr_nb(K, d - 1, A.cnz, A.bcz);
+    }
+    // x-stage: X[s][dj][dk] = lerp_x(e[I], e[I -/+ 1]) on the 3x3 (J,K) neighbourhood
+    double X[2][3][3];
+#pragma unroll
+    for (int dk = 0; dk < 3; ++dk) {
+#pragma unroll
+        for (int dj = 0; dj < 3; ++dj) {
+            const double *row = A.e + (size_t)A.cnx * ((size_t)yj[dj] + (size_t)A.cny * (size_t)zk[dk]);
+            const double em = __ldg(row + xi[0]), ec = __ldg(row + xi[1]), ep = __ldg(row + xi[2]);
+            X[0][dj][dk] = lerp(ec, em);
+            X[1][dj][dk] = lerp(ec, ep);
+        }
+    }
+    const size_t fplane = (size_t)A.nx * A.ny;
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+            double v[2];
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                // y-stage at the centre and at the far z plane, then the z-stage
+                const double yc = lerp(X[s][1][1], X[s][t ? 2 : 0][1]);
+                const double yf = lerp(X[s][1][u ? 2 : 0], X[s][t ? 2 : 0][u ? 2 : 0]);
+                v[s] = lerp(yc, yf);
+            }
+            const size_t c = (size_t)(2 * I) + (size_t)A.nx * (size_t)(2 * J + t) + fplane * (size_t)(2 * K + u);
+            const double2 pi = __ldg(reinterpret_cast<const double2 *>(A.pin + c));
+            double2 po;
+            po.x = __dadd_rn(pi.x, v[0]);
+            po.y = __dadd_rn(pi.y, v[1]);
+            *reinterpret_cast<double2 *>(A.pout + c) = po;
+        }
+    }
+}
+
+} // namespace mg
