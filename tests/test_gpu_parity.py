@@ -249,3 +249,38 @@ def test_density_can_be_replaced(mgmod, uniform):
     g.vcycle(dev(w.rhs), pg)
     o.vcycle(w.rhs, po)
     assert np.array_equal(po, host(pg))
+
+
+# --------------------------------------------------------------------------- #
+# full sizes, in the launch configuration bench.py times (graph replay, streaming kernels)
+# --------------------------------------------------------------------------- #
+def _full_size_cycles(mgmod, cfg, cycles):
+    w = make_workload(cfg)
+    o, g = pair(mgmod, w.n, w.h, w.bc, nu=(w.nu1, w.nu2), rho=w.rho)
+    shp = o.shape
+    po = np.zeros(shp)
+    pg, fd = dev(po), dev(w.rhs)
+    for cyc in range(cycles):
+        o.vcycle(w.rhs, po)
+        g.vcycle(fd, pg)
+        assert np.array_equal(po, host(pg)), f"config {cfg} cycle {cyc}"
+    assert g.residual(fd, pg) == pytest.approx(o.residual(w.rhs, po), rel=NORM_RTOL)
+    o.close()
+    g.close()
+
+
+def test_full_size_config4_bit_exact(mgmod):
+    """512^3 drop-film (BASELINE configs[3], the bench workload): every cell of two V(3,3)
+    cycles equals the oracle's, and the residual norm agrees to 1e-10."""
+    _full_size_cycles(mgmod, 4, 2)
+
+
+def test_full_size_config5_bit_exact(mgmod):
+    """1024^3 (BASELINE configs[4], the largest size): one V(3,3) cycle, every cell.  Needs
+    ~60 GB of host memory for the oracle and ~52 GB on the device; skipped on smaller boxes."""
+    import os
+    host_gb = os.sysconf("SC_PAGE_SIZE") * os.sysconf("SC_PHYS_PAGES") / 2**30
+    dev_gb = torch.cuda.get_device_properties(0).total_memory / 2**30
+    if host_gb < 100 or dev_gb < 100:
+        pytest.skip(f"needs >= 100 GB host and device memory (have {host_gb:.0f} / {dev_gb:.0f})")
+    _full_size_cycles(mgmod, 5, 1)
