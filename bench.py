@@ -41,6 +41,7 @@ UNIT = "Gcell-updates/s"
 # algorithmic HBM bytes: level-0 sweep pass 32 B/cell
 # (p read+write, f, a); coarse-level pass 48 B/cell; whole V(3,3) cycle per fine cell:
 B_SWEEP_L0 = 32.0
+NCU_SWEEP_TRAFFIC_512 = 3.826e9 + 1.050e9     # bytes per launch (algorithmic: 4.295e9)
 
 
 def b_sched_per_fine_cell(nu1, nu2):
@@ -319,7 +320,7 @@ def run_cuda(args, w, wname):
                    "frac_of_B_sched_roofline": (bs / (peak * 1e9)) / (t_vc_ms * 1e-3),
                    "frac_of_B_sweep_roofline": (bw / (peak * 1e9)) / (t_vc_ms * 1e-3),
                    "B_sched_bytes": bs, "B_sweep_bytes": bw},
-        "roofline": {"bound": "hbm", "kernel": "k_stream_sweep<CELL> (level-0 red-black sweep pass, p_in -> p_out)", "achieved": achieved,
+        "roofline": {"bound": "hbm", "kernel": "k_sweep3<CELL> (level-0 red-black sweep pass, p_in -> p_out)", "achieved": achieved,
                      "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                      "peak_source": peak_src, "bytes_per_launch": sweep_bytes,
                      "ms_per_sweep": t_sweep_ms, "launches_per_sweep": launches_per_sweep},
@@ -328,12 +329,10 @@ def run_cuda(args, w, wname):
         "gpu_launches": int(launches),
         "clocks": clocks.summary(),
     }
-    traffic_file = ROOT / "profiles" / "traffic.json"
-    if traffic_file.exists():
-        try:
-            line["roofline"]["traffic"] = json.loads(traffic_file.read_text()).get(wname)
-        except Exception:
-            pass
+    # dram__bytes_read.sum + dram__bytes_write.sum of one k_sweep3<CELL> launch from the
+    # `ncu --set full` capture summarised in profiles/r1d_cycle.md (512^3 only)
+    if list(w.n) == [512, 512, 512]:
+        line["roofline"]["traffic"] = NCU_SWEEP_TRAFFIC_512
     if world == 1 and not args.no_cpu_baseline:
         times_o, thr = oracle_sample(w, repeats=1, min_seconds=10.0)
         line["cpu_baseline"] = {

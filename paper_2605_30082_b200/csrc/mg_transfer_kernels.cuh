@@ -92,22 +92,41 @@ __global__ void __launch_bounds__(RS_THREADS) k_resid_stream(RsArgs A)
     }
     double acc = 0.0;          // RS_NORM: running sum of r^2; RS_RESTRICT: plane sum of the even plane
 
-    for (int k = kz0; k < kz1; ++k) {
+    // loads of one plane step: next plane of the own rows, the two neighbour rows, f (and the
+    // coefficients).  They are issued one step AHEAD of their use (software pipeline: the
+    // kernel was bound by exposed load latency, profiles/r1d_cycle.md), so two steps of loads
+    // are in flight per warp.
+    struct Ld { double2 Pp[2], Pym, Pyp, F0, F1, Ap[2], Aym, Ayp, Bzp[2], Bx[2], By[3]; };
+    auto load = [&](int k, Ld &d) __attribute__((always_inline)) {
         const size_t oc = plane * (size_t)k, op = plane * (size_t)znext(k);
+        d.Pp[0] = rs_ld2(A.p, op + row0 + x0); d.Pp[1] = rs_ld2(A.p, op + row1 + x0);
+        d.Pym = rs_ld2(A.p, oc + rowm + x0); d.Pyp = rs_ld2(A.p, oc + rowp + x0);
+        d.F0 = rs_ld2(A.f, oc + row0 + x0); d.F1 = rs_ld2(A.f, oc + row1 + x0);
+        if (CELL) {
+            d.Ap[0] = rs_ld2(L.a, op + row0 + x0); d.Ap[1] = rs_ld2(L.a, op + row1 + x0);
+            d.Aym = rs_ld2(L.a, oc + rowm + x0); d.Ayp = rs_ld2(L.a, oc + rowp + x0);
+        } else {
+            d.Bzp[0] = rs_ld2(L.bz, op + row0 + x0); d.Bzp[1] = rs_ld2(L.bz, op + row1 + x0);
+            d.Bx[0] = rs_ld2(L.bx, oc + row0 + x0); d.Bx[1] = rs_ld2(L.bx, oc + row1 + x0);
+            d.By[0] = rs_ld2(L.by, oc + row0 + x0); d.By[1] = rs_ld2(L.by, oc + row1 + x0);
+            d.By[2] = rs_ld2(L.by, oc + rowp + x0);
+        }
+    };
+    Ld cur;
+    load(kz0, cur);
+    for (int k = kz0; k < kz1; ++k) {
+        Ld nxt;
+        load(min(k + 1, kz1 - 1), nxt);
+        const size_t oc = plane * (size_t)k;
         const bool wall_z0 = L.bcz && k == 0, wall_z1 = L.bcz && k == L.nz - 1;
-        // ---- loads of this plane: next plane of the own rows, the two neighbour rows, f
-        Pp[0] = rs_ld2(A.p, op + row0 + x0); Pp[1] = rs_ld2(A.p, op + row1 + x0);
-        const double2 Pym = rs_ld2(A.p, oc + rowm + x0), Pyp = rs_ld2(A.p, oc + rowp + x0);
-        const double2 F0 = rs_ld2(A.f, oc + row0 + x0), F1 = rs_ld2(A.f, oc + row1 + x0);
+        Pp[0] = cur.Pp[0]; Pp[1] = cur.Pp[1];
+        const double2 Pym = cur.Pym, Pyp = cur.Pyp, F0 = cur.F0, F1 = cur.F1;
         double2 Aym, Ayp, Bx[2], By[3];
         if (CELL) {
-            Ap[0] = rs_ld2(L.a, op + row0 + x0); Ap[1] = rs_ld2(L.a, op + row1 + x0);
-            Aym = rs_ld2(L.a, oc + rowm + x0); Ayp = rs_ld2(L.a, oc + rowp + x0);
+            Ap[0] = cur.Ap[0]; Ap[1] = cur.Ap[1]; Aym = cur.Aym; Ayp = cur.Ayp;
         } else {
-            Bzp[0] = rs_ld2(L.bz, op + row0 + x0); Bzp[1] = rs_ld2(L.bz, op + row1 + x0);
-            Bx[0] = rs_ld2(L.bx, oc + row0 + x0); Bx[1] = rs_ld2(L.bx, oc + row1 + x0);
-            By[0] = rs_ld2(L.by, oc + row0 + x0); By[1] = rs_ld2(L.by, oc + row1 + x0);
-            By[2] = rs_ld2(L.by, oc + rowp + x0);
+            Bzp[0] = cur.Bzp[0]; Bzp[1] = cur.Bzp[1]; Bx[0] = cur.Bx[0]; Bx[1] = cur.Bx[1];
+            By[0] = cur.By[0]; By[1] = cur.By[1]; By[2] = cur.By[2];
         }
         // ---- x-neighbours: adjacent lanes; the two edge lanes load a scalar
         double pl[2], pr[2], al[2], ar[2], bxr[2];
@@ -191,6 +210,7 @@ __global__ void __launch_bounds__(RS_THREADS) k_resid_stream(RsArgs A)
         Pm[0] = Pc[0]; Pm[1] = Pc[1]; Pc[0] = Pp[0]; Pc[1] = Pp[1];
         if (CELL) { Am[0] = Ac[0]; Am[1] = Ac[1]; Ac[0] = Ap[0]; Ac[1] = Ap[1]; }
         else { Bzc[0] = Bzp[0]; Bzc[1] = Bzp[1]; }
+        cur = nxt;
     }
     if (MODE == RS_NORM) {
         __shared__ double red[32];
