@@ -171,6 +171,20 @@ def run_reference(args, w, wname):
 # ------------------------------------------------------------------------------------
 # CUDA arm
 # ------------------------------------------------------------------------------------
+def aggregate_replicas(times_ms, counts, dist, device):
+    """Replicas only: every rank times its own independent solves.  The job's
+    time is the MAX over ranks, its work the SUM over ranks; no other collective touches the
+    data path.  `dist` is torch.distributed or None (single process)."""
+    import torch
+
+    t = torch.tensor(list(times_ms), dtype=torch.float64, device=device)
+    c = torch.tensor(list(counts), dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return t.tolist(), c.tolist()
+
+
 def run_cuda(args, w, wname):
     import torch
 
@@ -285,14 +299,9 @@ def run_cuda(args, w, wname):
         barrier()
         t_e2e_ms = ev0.elapsed_time(ev1)
 
-    # max over ranks
-    times = torch.tensor([t_ms, t_e2e_ms], dtype=torch.float64, device=devname)
-    counts = torch.tensor([float(cycles_total), float(e2e_cycles)], dtype=torch.float64, device=devname)
-    if dist is not None:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-        dist.all_reduce(counts, op=dist.ReduceOp.SUM)
-    t_ms, t_e2e_ms = times.tolist()
-    cycles_all, e2e_cycles_all = counts.tolist()
+    # max over ranks of the times, sum over ranks of the units
+    (t_ms, t_e2e_ms), (cycles_all, e2e_cycles_all) = aggregate_replicas(
+        [t_ms, t_e2e_ms], [float(cycles_total), float(e2e_cycles)], dist, devname)
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
