@@ -395,6 +395,65 @@ int mgo_solve(mgo_solver *s, const double *rhs, double *p, double rtol, int max_
     return status;
 }
 
+/* ------------------------------------------------- projection steps (S8(f) rank 2) */
+/* The two steps either side of the pressure solve in the projection method implied by
+ * P:33-36 (eq. 1-2) and stated in BJ:north_star: the right-hand side div(u*)/dt from the
+ * staggered intermediate velocity, and the correction u = u* - dt * beta_face * grad p.
+ * Staggering (R21): u[i,j,k] lives on the MINUS x-face of cell (i,j,k) (the face bx[i,j,k]
+ * belongs to), v on the minus y-face, w on the minus z-face; the plus face of a cell is the
+ * next cell's minus face (wrap).  On a Neumann axis the wrap face is the wall (both walls
+ * share the entry) and the caller supplies u = 0 there; its beta is 0, so the correction
+ * never changes it.
+ *   C10  s = 1.0/(h*dt);  f = (((u[i+1]-u[i]) + (v[j+1]-v[j])) + (w[k+1]-w[k])) * s
+ *   C11  g = dt/h;        u[i] = fma(-g, bx[i]*(p[i]-p[i-1]), u[i])   (v, w alike)
+ * Then div(u_new)/dt = f - A p cell by cell (pinned), i.e. the projected field is
+ * divergence-free to the residual of the solve. */
+int mgo_project_rhs(const mgo_solver *s, const double *u, const double *v, const double *w,
+                    double dt, double *f)
+{
+    if (!s || !u || !v || !w || !f || !(dt > 0.0) || !isfinite(dt)) return MGO_EINVAL;
+    const level_t *L = &s->lv[0];
+    const int nx = L->nx, ny = L->ny, nz = L->nz;
+    const double hd = L->h * dt;
+    const double sc = 1.0 / hd;
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                const int ip = i == nx - 1 ? 0 : i + 1;
+                const int jp = j == ny - 1 ? 0 : j + 1;
+                const int kp = k == nz - 1 ? 0 : k + 1;
+                const size_t c = IDX(L, i, j, k);
+                const double du = u[IDX(L, ip, j, k)] - u[c];
+                const double dv = v[IDX(L, i, jp, k)] - v[c];
+                const double dw = w[IDX(L, i, j, kp)] - w[c];
+                f[c] = ((du + dv) + dw) * sc;
+            }
+    return MGO_OK;
+}
+
+int mgo_project_correct(const mgo_solver *s, const double *p, double dt, double *u, double *v, double *w)
+{
+    if (!s || !u || !v || !w || !p || !(dt > 0.0) || !isfinite(dt)) return MGO_EINVAL;
+    const level_t *L = &s->lv[0];
+    const int nx = L->nx, ny = L->ny, nz = L->nz;
+    const double g = dt / L->h;
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                const int im = i == 0 ? nx - 1 : i - 1;
+                const int jm = j == 0 ? ny - 1 : j - 1;
+                const int km = k == 0 ? nz - 1 : k - 1;
+                const size_t c = IDX(L, i, j, k);
+                const double pc = p[c];
+                u[c] = fma(-g, L->bx[c] * (pc - p[IDX(L, im, j, k)]), u[c]);
+                v[c] = fma(-g, L->by[c] * (pc - p[IDX(L, i, jm, k)]), v[c]);
+                w[c] = fma(-g, L->bz[c] * (pc - p[IDX(L, i, j, km)]), w[c]);
+            }
+    return MGO_OK;
+}
+
 /* ------------------------------------------------------- step-level access */
 int mgo_num_levels(const mgo_solver *s) { return s ? s->nlev : MGO_EINVAL; }
 

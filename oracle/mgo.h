@@ -57,6 +57,15 @@ int  mgo_residual(mgo_solver *s, const double *rhs, const double *p, double *r_o
 int  mgo_solve(mgo_solver *s, const double *rhs, double *p, double rtol, int max_cycles,
                int *cycles_out, double *relres_out, double *hist_or_null);
 
+/* ---- projection steps either side of the solve (staggering and the
+ * expression trees C10, C11 are stated in mgo.c) ----
+ * f = div(u*)/dt from the staggered velocity (u,v,w on the minus faces of each cell) */
+int  mgo_project_rhs(const mgo_solver *s, const double *u, const double *v, const double *w,
+                     double dt, double *f);
+/* u -= dt * beta_face * grad p, in place, with the level-0 face coefficients */
+int  mgo_project_correct(const mgo_solver *s, const double *p, double dt, double *u, double *v,
+                         double *w);
+
 /* ---- step-level entry points (used by the pins and by step-by-step parity) ---- */
 int  mgo_num_levels(const mgo_solver *s);
 int  mgo_level_dims(const mgo_solver *s, int level, int dims[3], double *h_level);

@@ -77,6 +77,8 @@ def lib():
         L.mgo_residual_level.argtypes = [vp, C.c_int, dp, dp, dp]
         L.mgo_restrict.argtypes = [vp, C.c_int, dp, dp]
         L.mgo_prolong_add.argtypes = [vp, C.c_int, dp, dp]
+        L.mgo_project_rhs.argtypes = [vp, dp, dp, dp, C.c_double, dp]
+        L.mgo_project_correct.argtypes = [vp, dp, C.c_double, dp, dp, dp]
         L.mgo_threads.restype = C.c_int
         L.mgo_set_threads.argtypes = [C.c_int]
         L.mgo_set_threads.restype = None
@@ -176,6 +178,19 @@ class Oracle:
         if st < 0:
             raise OracleError(st)
         return st, cyc.value, rel.value, hist[: cyc.value + 1].copy()
+
+    # ---- projection steps
+    def project_rhs(self, u, v, w, dt):
+        f = np.empty(self.shape)
+        _chk(lib().mgo_project_rhs(self._h, _dp(self._arr(u)), _dp(self._arr(v)), _dp(self._arr(w)),
+                                   float(dt), _dp(f)))
+        return f
+
+    def project_correct(self, p, dt, u, v, w):
+        for a in (u, v, w):
+            assert a.flags["C_CONTIGUOUS"] and a.dtype == np.float64 and a.shape == self.shape
+        _chk(lib().mgo_project_correct(self._h, _dp(self._arr(p)), float(dt), _dp(u), _dp(v), _dp(w)))
+        return u, v, w
 
     # ---- step level
     def faces(self, level):
