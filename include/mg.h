@@ -132,6 +132,28 @@ int mg_solve_host(mg_handle *s, const double *rho_host, const double *rhs_host, 
                   double rtol, int max_cycles, int *cycles_host, double *relres_host,
                   double *hist_host);
 
+/* ---- projection steps either side of the solve (eq. 1-2).
+ * Staggered velocity: u_dev[i,j,k] is the component on the MINUS x-face of cell (i,j,k) (the
+ * face between cells (i-1,j,k) and (i,j,k)), v_dev on the minus y-face, w_dev on the minus
+ * z-face; N doubles each, x fastest; a cell's plus face is the next cell's minus face (wrap).
+ * On a Neumann axis the wrap face is the wall and the caller keeps the velocity there at 0.
+ *
+ * mg_project_rhs:     f = ((u[i+1]-u[i]) + (v[j+1]-v[j]) + (w[k+1]-w[k])) / (h dt)
+ * mg_project_correct: u[i] -= (dt/h) beta_x[i] (p[i]-p[i-1]), likewise v, w, with the level-0
+ *                     face coefficients of the current density (wall faces: beta = 0).
+ * mg_project:         rhs -> mg_solve (p_dev: in = initial guess) -> correct; rhs_dev is N
+ *                     doubles of caller-owned scratch that receives the right-hand side.
+ * After mg_project the discrete divergence of (u,v,w) equals dt x the final residual.
+ * All asynchronous on the stream except mg_project (mg_solve synchronises).
+ * Errors: MG_EINVAL (NULL pointer, dt <= 0 or non-finite); mg_project also mg_solve's codes
+ * (on a negative status the velocity is left untouched). */
+int mg_project_rhs(mg_handle *s, const double *u_dev, const double *v_dev, const double *w_dev,
+                   double dt, double *f_dev);
+int mg_project_correct(mg_handle *s, const double *p_dev, double dt, double *u_dev, double *v_dev,
+                       double *w_dev);
+int mg_project(mg_handle *s, double *u_dev, double *v_dev, double *w_dev, double dt, double *p_dev,
+               double *rhs_dev, double rtol, int max_cycles, int *cycles_host, double *relres_host);
+
 const char *mg_strerror(int status);
 /* Text of the last CUDA error seen by this thread inside the library ("" if none). */
 const char *mg_last_cuda_error(void);

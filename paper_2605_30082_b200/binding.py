@@ -33,6 +33,9 @@ SIGNATURES = {
     "mg_residual": (C.c_int, [_vp, _dp, _dp, _dp, _hp]),
     "mg_solve": (C.c_int, [_vp, _dp, _dp, C.c_double, C.c_int, _ip, _hp, _hp]),
     "mg_solve_host": (C.c_int, [_vp, _vp, _vp, _vp, C.c_double, C.c_int, _ip, _hp, _hp]),
+    "mg_project_rhs": (C.c_int, [_vp, _dp, _dp, _dp, C.c_double, _dp]),
+    "mg_project_correct": (C.c_int, [_vp, _dp, C.c_double, _dp, _dp, _dp]),
+    "mg_project": (C.c_int, [_vp, _dp, _dp, _dp, C.c_double, _dp, _dp, C.c_double, C.c_int, _ip, _hp]),
     "mg_strerror": (C.c_char_p, [C.c_int]),
     "mg_last_cuda_error": (C.c_char_p, []),
     "mg_num_levels": (C.c_int, [_vp]),
@@ -193,6 +196,26 @@ class Multigrid:
         if st < 0:
             raise MgError(st)
         return st, cyc.value, rel.value, list(hist[: cyc.value + 1])
+
+    # ---- projection steps either side of the solve
+    def project_rhs(self, u, v, w, dt, f):
+        _chk(lib().mg_project_rhs(self._h, _ptr(u, self.shape), _ptr(v, self.shape), _ptr(w, self.shape),
+                                  float(dt), _ptr(f, self.shape)))
+        return f
+
+    def project_correct(self, p, dt, u, v, w):
+        _chk(lib().mg_project_correct(self._h, _ptr(p, self.shape), float(dt), _ptr(u, self.shape),
+                                      _ptr(v, self.shape), _ptr(w, self.shape)))
+
+    def project(self, u, v, w, dt, p, rhs, rtol, max_cycles):
+        """rhs -> solve -> correct; returns (status, cycles, relres)."""
+        cyc, rel = C.c_int(), C.c_double()
+        st = lib().mg_project(self._h, _ptr(u, self.shape), _ptr(v, self.shape), _ptr(w, self.shape), float(dt),
+                              _ptr(p, self.shape), _ptr(rhs, self.shape), float(rtol), int(max_cycles),
+                              C.byref(cyc), C.byref(rel))
+        if st < 0:
+            raise MgError(st)
+        return st, cyc.value, rel.value
 
     # ---- single steps
     def level_faces(self, level):
