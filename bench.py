@@ -284,6 +284,52 @@ def run_cuda(args, w, wname):
         torch.cuda.synchronize()
         t_setrho_ms = ev0.elapsed_time(ev1)
 
+        # the projection step around the solve: rhs = div(u*)/dt,
+        # solve, u -= dt beta grad p, on the 16-mode staggered velocity behind the workload's rhs
+        proj = None
+        if args.projection and getattr(w, "seed", None) is not None and tuple(w.bc) == (0, 0, 1):
+            from workloads import velocity_field
+            uh, vh, wh = velocity_field(w.n, w.h, w.seed)
+            u0, v0, w0 = (torch.from_numpy(a).to(devname) for a in (uh, vh, wh))
+            del uh, vh, wh
+            ud, vd, wd = u0.clone(), v0.clone(), w0.clone()
+            fd = torch.empty_like(p_d)
+            dtp = 1.0
+            for _ in range(2):
+                g.project_rhs(ud, vd, wd, dtp, fd)
+                g.project_correct(p_d, dtp, ud, vd, wd)
+            torch.cuda.synchronize()
+            ev0.record(stream)
+            for _ in range(10):
+                g.project_rhs(ud, vd, wd, dtp, fd)
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            t_rhs = ev0.elapsed_time(ev1) / 10
+            ev0.record(stream)
+            for _ in range(10):
+                g.project_correct(p_d, dtp, ud, vd, wd)
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            t_cor = ev0.elapsed_time(ev1) / 10
+            ud.copy_(u0); vd.copy_(v0); wd.copy_(w0)
+            p_d.zero_()
+            torch.cuda.synchronize()
+            ev0.record(stream)
+            pst, pcyc, prel = g.project(ud, vd, wd, dtp, p_d, fd, w.rtol, max_cycles)
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            t_proj = ev0.elapsed_time(ev1)
+            g.project_rhs(ud, vd, wd, dtp, fd)
+            div_after = float(torch.linalg.vector_norm(fd))
+            g.project_rhs(u0, v0, w0, dtp, fd)
+            div_before = float(torch.linalg.vector_norm(fd))
+            proj = {"ms_per_step": t_proj, "cycles": pcyc, "relres": prel, "status": pst,
+                    "rhs_ms": t_rhs, "rhs_gbs": 32.0 * N / (t_rhs * 1e-3) / 1e9,
+                    "correct_ms": t_cor, "correct_gbs": 64.0 * N / (t_cor * 1e-3) / 1e9,
+                    "div_after_over_before": div_after / div_before,
+                    "what": "mg_project = rhs (32 B/cell) + mg_solve + correct (64 B/cell), dt = 1"}
+            del u0, v0, w0, ud, vd, wd, fd
+
         # end to end from pinned host buffers through mg_solve_host
         rho_h = torch.from_numpy(w.rho).pin_memory()
         rhs_h = torch.from_numpy(w.rhs).pin_memory()
@@ -338,6 +384,8 @@ def run_cuda(args, w, wname):
         "gpu_launches": int(launches),
         "clocks": clocks.summary(),
     }
+    if proj is not None:
+        line["projection_step"] = proj
     # dram__bytes_read.sum + dram__bytes_write.sum of one k_sweep3<CELL> launch from the
     # `ncu --set full` capture summarised in profiles/r1d_cycle.md (512^3 only)
     if list(w.n) == [512, 512, 512]:
@@ -361,6 +409,8 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="config4", help="config<k>[@n], k = 1..5 (BASELINE.json configs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-projection", dest="projection", action="store_false",
+                    help="skip the projection-step timing (rhs + solve + correct)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3

@@ -75,3 +75,20 @@ def test_generation_is_reproducible():
     assert np.array_equal(a.rho, b.rho) and np.array_equal(a.rhs, b.rhs)
     assert not np.array_equal(make_workload(2, 32).rhs, make_workload(3, 32).rhs)
     assert set(CONFIGS) == {1, 2, 3, 4, 5}
+
+
+def test_velocity_field_reproduces_the_rhs_of_config3():
+    """The materialised 16-mode staggered velocity is the field behind the workload's rhs:
+    its divergence (oracle C10, dt = 1) equals rhs up to rounding and the removed mean, and it
+    has closed walls in z."""
+    import numpy as np
+    from oracle.mgo import Oracle
+    from workloads import make_workload, velocity_field
+
+    w = make_workload(3, 32)
+    u, v, ww = velocity_field(w.n, w.h, w.seed)
+    assert np.all(ww[0] == 0.0)
+    o = Oracle(w.n, w.h, w.bc)
+    f = o.project_rhs(u, v, ww, 1.0)
+    f -= f.mean()
+    assert np.abs(f - w.rhs).max() <= 1e-10 * np.abs(w.rhs).max()

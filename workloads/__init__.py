@@ -16,4 +16,5 @@ from .configs import (  # noqa: F401
     Workload,
     make_workload,
     splitmix64_uniform,
+    velocity_field,
 )

@@ -197,6 +197,46 @@ def _rhs_velocity_divergence(n, h, seed, nmodes=16):
     return _remove_mean(f)
 
 
+def velocity_field(n, h, seed, nmodes=16):
+    """The staggered velocity behind _rhs_velocity_divergence, materialised: u on the minus
+    x-faces, v on the minus y-faces, w on the minus z-faces of every cell (w = 0 on the bottom
+    wall k = 0, which is also the top wall of the wrapped array).  Same seed stream, same modes;
+    input for the projection steps (mg_project_rhs with dt = 1 reproduces the workload's rhs up
+    to rounding and the removed mean).  Returns (u, v, w), each (nz, ny, nx) fp64."""
+    nx, ny, nz = n
+    st = _Stream(seed)
+    xi_f = np.arange(nx) * h
+    xi_c = (np.arange(nx) + 0.5) * h
+    yj_f = np.arange(ny) * h
+    yj_c = (np.arange(ny) + 0.5) * h
+    zk_c = (np.arange(nz) + 0.5) * h
+    two_pi = 2.0 * math.pi
+    u = np.zeros((nz, ny, nx), dtype=np.float64)
+    v = np.zeros_like(u)
+    w = np.zeros_like(u)
+    chunk = 8
+    for _ in range(nmodes):
+        kx = st.integer(-4, 4)
+        ky = st.integer(-4, 4)
+        kz = st.integer(1, 4)
+        phi = two_pi * float(st.uniform()[0])
+        ax = st.real(-1.0, 1.0)
+        ay = st.real(-1.0, 1.0)
+        az = st.real(-1.0, 1.0)
+        ux = ax * np.cos(two_pi * (kx * xi_f[None, :] + ky * yj_c[:, None]) + phi)
+        vy = ay * np.cos(two_pi * (kx * xi_c[None, :] + ky * yj_f[:, None]) + phi)
+        wc = az * np.cos(two_pi * (kx * xi_c[None, :] + ky * yj_c[:, None]) + phi)
+        cz = np.cos(math.pi * kz * zk_c)
+        sz = np.sin(math.pi * kz * np.arange(nz) * h)      # minus z-face of plane k is at z = k h
+        sz[0] = 0.0
+        for k0 in range(0, nz, chunk):
+            k1 = min(nz, k0 + chunk)
+            u[k0:k1] += ux[None, :, :] * cz[k0:k1, None, None]
+            v[k0:k1] += vy[None, :, :] * cz[k0:k1, None, None]
+            w[k0:k1] += wc[None, :, :] * sz[k0:k1, None, None]
+    return u, v, w
+
+
 # --------------------------------------------------------------------------- #
 # the five configs
 # --------------------------------------------------------------------------- #
