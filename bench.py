@@ -330,6 +330,33 @@ def run_cuda(args, w, wname):
                     "what": "mg_project = rhs (32 B/cell) + mg_solve + correct (64 B/cell), dt = 1"}
             del u0, v0, w0, ud, vd, wd, fd
 
+        # optional: a time sequence: the drop falls onto the film, the density
+        # changes every step (set_density), the solve is warm-started from the previous pressure
+        seq = None
+        if args.sequence > 0 and tuple(w.bc) == (0, 0, 1):
+            from workloads import sequence_density
+            cfg_id, n_over = parse_workload(args.workload)
+            rows = []
+            p_d.zero_()
+            for sidx in range(args.sequence):
+                rho_s = torch.from_numpy(sequence_density(cfg_id, n_over, sidx, args.sequence)).to(devname)
+                torch.cuda.synchronize()
+                ev0.record(stream)
+                g.set_density(rho_s)
+                ev1.record(stream)
+                torch.cuda.synchronize()
+                t_sd = ev0.elapsed_time(ev1)
+                ev0.record(stream)
+                st_s, cyc_s, rel_s, _ = g.solve(rhs_d, p_d, w.rtol, max_cycles)      # warm start
+                ev1.record(stream)
+                torch.cuda.synchronize()
+                rows.append({"step": sidx, "set_density_ms": t_sd, "solve_ms": ev0.elapsed_time(ev1),
+                             "cycles": cyc_s, "status": st_s})
+                del rho_s
+            seq = {"steps": rows, "what": "drop centre falls 0.8 r onto its config position in equal steps; "
+                   "rhs fixed; p warm-started from the previous step (step 0 from p = 0)"}
+            g.set_density(rho_d)
+
         # end to end from pinned host buffers through mg_solve_host
         rho_h = torch.from_numpy(w.rho).pin_memory()
         rhs_h = torch.from_numpy(w.rhs).pin_memory()
@@ -386,6 +413,8 @@ def run_cuda(args, w, wname):
     }
     if proj is not None:
         line["projection_step"] = proj
+    if seq is not None:
+        line["time_sequence"] = seq
     # dram__bytes_read.sum + dram__bytes_write.sum of one k_sweep3<CELL> launch from the
     # `ncu --set full` capture summarised in profiles/r1d_cycle.md (512^3 only)
     if list(w.n) == [512, 512, 512]:
@@ -409,6 +438,8 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="config4", help="config<k>[@n], k = 1..5 (BASELINE.json configs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sequence", type=int, default=0,
+                    help="also run a K-step falling-drop sequence (set_density + warm-started solve per step)")
     ap.add_argument("--no-projection", dest="projection", action="store_false",
                     help="skip the projection-step timing (rhs + solve + correct)")
     args = ap.parse_args()

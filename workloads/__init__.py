@@ -15,6 +15,7 @@ from .configs import (  # noqa: F401
     CONFIGS,
     Workload,
     make_workload,
+    sequence_density,
     splitmix64_uniform,
     velocity_field,
 )

@@ -285,3 +285,16 @@ def make_workload(config: int, n: Optional[int] = None) -> Workload:
         raise KeyError(config)
     return Workload(name, shape, h, c["bc"], rho, rhs, nu1, nu2, c["rtol"],
                     seed=c["seed"], note=c["what"])
+
+
+def sequence_density(config: int, n: Optional[int], step: int, nsteps: int) -> np.ndarray:
+    """Density of time step `step` (0 .. nsteps-1) of a drop falling onto the film (the paper's
+    subject): the geometry of configs 3-5 with the drop
+    centre starting 0.8 radii above its config position and ending exactly there, in equal
+    steps.  Same sub-sampling and mixing as the configs (R19); seeded by nothing (closed form)."""
+    assert config in (3, 4, 5) and 0 <= step < nsteps
+    c = CONFIGS[config]
+    nn = int(n if n is not None else c["n"])
+    film, r, cz = (0.10, 0.10, 0.15) if config in (3, 4) else (0.05, 0.05, 0.10)
+    lift = 0.8 * r * (1.0 - step / max(1, nsteps - 1))
+    return _mixed_density((nn, nn, nn), 1.0 / nn, 1.2, film, 935.0, (0.5, 0.5, cz + lift), r, 998.0)
