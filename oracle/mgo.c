@@ -395,6 +395,193 @@ int mgo_solve(mgo_solver *s, const double *rhs, double *p, double rtol, int max_
     return status;
 }
 
+/* ----------------------------------------- MG-preconditioned CG (S8(f) rank 1) */
+/* R22.  The V-cycle of mgo_vcycle is not a symmetric operator: its post-smoothing repeats the
+ * red->black order and its restriction (8-child mean, R11) is not a multiple of the transpose
+ * of its prolongation (trilinear, R12).  The preconditioner M of the CG solver is the
+ * SYMMETRIC cycle: nu1 red->black sweeps, residual, restriction R' = (1/8) P^T (the transpose
+ * of the trilinear prolongation, i.e. the other "full-weighting" reading of R11), coarse
+ * correction from zero, prolongation P, nu2 = nu1 black->red sweeps; coarsest level:
+ * coarse_sweeps red->black then coarse_sweeps black->red sweeps.  z = M r starts from z = 0.
+ *   C14  R'  per axis, x then y then z:  t = w0*r0; t = fma(w1,r1,t); t = fma(w2,r2,t);
+ *        t = fma(w3,r3,t) over the fine indices 2I-1, 2I, 2I+1, 2I+2 (wrapped; absent beyond a
+ *        Neumann wall: weight 0), w_q = 0.75 [near(i_q) = I] + 0.25 [far(i_q) = I] with near,
+ *        far as in C8; finally fc = 0.125 * t.
+ *   C12  A d = ih2 * fma(-D, d, S)
+ *   C13  PCG (A, M negative definite on the zero-mean subspace; the formulas need no sign):
+ *        r = f - A p ; z = M r ; d = z ; rz = r.z ; then per iteration
+ *        q = A d ; alpha = rz / (d.q) ; p = fma(alpha,d,p) ; r = fma(-alpha,q,r) ;
+ *        stop when ||r|| <= rtol ||r_0|| (r from the recurrence) ;
+ *        z = M r ; rz' = r.z ; beta = rz'/rz ; d = fma(beta,d,z).
+ *        dot products as C9 (any order, accurate to ~1e-15); mean of p removed at the end. */
+static void sweep_rev(const level_t *L, const double *f, double *p)
+{
+    smooth_half(L, 1, f, p);
+    smooth_half(L, 0, f, p);
+}
+
+/* weight of coarse index I in the prolongation row of fine index i (C8's near / far rule) */
+static inline double pt_weight(int i, int I, int cn, int neumann)
+{
+    const int near = i >> 1;
+    const int far = far_index(near, i & 1, cn, neumann);
+    return (near == I ? 0.75 : 0.0) + (far == I ? 0.25 : 0.0);
+}
+
+/* the four fine indices 2I-1 .. 2I+2 that can carry coarse index I, wrapped or (Neumann)
+ * clamped with weight 0 when they fall outside */
+static inline void pt_stencil(int I, int fn, int cn, int neumann, int idx[4], double w[4])
+{
+    for (int q = 0; q < 4; ++q) {
+        int i = 2 * I - 1 + q;
+        int outside = 0;
+        if (i < 0) { if (neumann) { outside = 1; i = 0; } else i += fn; }
+        if (i >= fn) { if (neumann) { outside = 1; i = fn - 1; } else i -= fn; }
+        idx[q] = i;
+        w[q] = outside ? 0.0 : pt_weight(i, I, cn, neumann);
+    }
+}
+
+static void restrict_adj(const mgo_solver *s, const level_t *F, const level_t *C, const double *r, double *fc)
+{
+#pragma omp parallel for schedule(static)
+    for (int K = 0; K < C->nz; ++K)
+        for (int J = 0; J < C->ny; ++J)
+            for (int I = 0; I < C->nx; ++I) {
+                int ix[4], iy[4], iz[4];
+                double wx[4], wy[4], wz[4];
+                pt_stencil(I, F->nx, C->nx, s->bc[0] == 1, ix, wx);
+                pt_stencil(J, F->ny, C->ny, s->bc[1] == 1, iy, wy);
+                pt_stencil(K, F->nz, C->nz, s->bc[2] == 1, iz, wz);
+                double tz = 0.0;
+                for (int c = 0; c < 4; ++c) {
+                    double ty = 0.0;
+                    for (int b = 0; b < 4; ++b) {
+                        double tx = wx[0] * r[IDX(F, ix[0], iy[b], iz[c])];
+                        tx = fma(wx[1], r[IDX(F, ix[1], iy[b], iz[c])], tx);
+                        tx = fma(wx[2], r[IDX(F, ix[2], iy[b], iz[c])], tx);
+                        tx = fma(wx[3], r[IDX(F, ix[3], iy[b], iz[c])], tx);
+                        ty = b == 0 ? wy[0] * tx : fma(wy[b], tx, ty);
+                    }
+                    tz = c == 0 ? wz[0] * ty : fma(wz[c], ty, tz);
+                }
+                fc[IDX(C, I, J, K)] = 0.125 * tz;
+            }
+}
+
+static void vcycle_sym(mgo_solver *s, int l, double *p, const double *f)
+{
+    level_t *L = &s->lv[l];
+    if (l == s->nlev - 1) {
+        for (int it = 0; it < s->coarse_sweeps; ++it) sweep(L, f, p);
+        for (int it = 0; it < s->coarse_sweeps; ++it) sweep_rev(L, f, p);
+        return;
+    }
+    level_t *C = &s->lv[l + 1];
+    for (int it = 0; it < s->nu1; ++it) sweep(L, f, p);
+    residual(L, f, p, L->r);
+    restrict_adj(s, L, C, L->r, C->f);
+    memset(C->p, 0, lv_cells(C) * sizeof(double));
+    vcycle_sym(s, l + 1, C->p, C->f);
+    prolong_add(s, L, C, C->p, p);
+    for (int it = 0; it < s->nu2; ++it) sweep_rev(L, f, p);
+}
+
+int mgo_restrict_adj(const mgo_solver *s, int level, const double *r, double *fc)
+{
+    if (!s || level < 0 || level >= s->nlev - 1 || !r || !fc) return MGO_EINVAL;
+    restrict_adj(s, &s->lv[level], &s->lv[level + 1], r, fc);
+    return MGO_OK;
+}
+
+/* z = M r: one symmetric cycle from z = 0 */
+int mgo_precondition(mgo_solver *s, const double *r, double *z)
+{
+    if (!s || !r || !z || s->nu1 != s->nu2) return MGO_EINVAL;
+    memset(z, 0, lv_cells(&s->lv[0]) * sizeof(double));
+    vcycle_sym(s, 0, z, r);
+    return MGO_OK;
+}
+
+static long double dot_planes(const level_t *L, const double *x, const double *y)
+{
+    long double *part = (long double *)malloc((size_t)L->nz * sizeof(long double));
+    size_t plane = (size_t)L->nx * L->ny;
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < L->nz; ++k) {
+        long double acc = 0.0L;
+        const double *a = x + plane * (size_t)k, *b = y + plane * (size_t)k;
+        for (size_t c = 0; c < plane; ++c) acc += (long double)a[c] * (long double)b[c];
+        part[k] = acc;
+    }
+    long double tot = 0.0L;
+    for (int k = 0; k < L->nz; ++k) tot += part[k];
+    free(part);
+    return tot;
+}
+
+int mgo_solve_pcg(mgo_solver *s, const double *rhs, double *p, double rtol, int max_iter,
+                  int *iters_out, double *relres_out, double *hist)
+{
+    if (!s || !rhs || !p || !(rtol >= 0.0) || max_iter < 0 || s->nu1 != s->nu2) return MGO_EINVAL;
+    level_t *L = &s->lv[0];
+    const size_t N = lv_cells(L);
+    {
+        long double mean = sum_planes(L, rhs, 0) / (long double)N;
+        long double nrm = sqrtl(sum_planes(L, rhs, 1));
+        if (fabsl(mean) > 1e-12L * (nrm / sqrtl((long double)N))) return MGO_EINCOMPATIBLE;
+    }
+    double *r = (double *)malloc(N * sizeof(double)), *z = (double *)malloc(N * sizeof(double));
+    double *d = (double *)malloc(N * sizeof(double)), *q = (double *)malloc(N * sizeof(double));
+    if (!r || !z || !d || !q) { free(r); free(z); free(d); free(q); return MGO_ENOMEM; }
+    residual(L, rhs, p, r);
+    const double r0 = (double)sqrtl(sum_planes(L, r, 1));
+    if (hist) hist[0] = r0;
+    int k = 0, status = MGO_NOT_CONVERGED;
+    double rk = r0;
+    if (!isfinite(r0)) status = MGO_EDIVERGED;
+    else if (r0 <= rtol * r0) status = MGO_OK;
+    double rz = 0.0;
+    if (status == MGO_NOT_CONVERGED && max_iter > 0) {
+        memset(z, 0, N * sizeof(double));
+        vcycle_sym(s, 0, z, r);
+        memcpy(d, z, N * sizeof(double));
+        rz = (double)dot_planes(L, r, z);
+    }
+    while (status == MGO_NOT_CONVERGED && k < max_iter) {
+        apply(L, d, q);
+        const double dq = (double)dot_planes(L, d, q);
+        const double alpha = rz / dq;
+#pragma omp parallel for schedule(static)
+        for (size_t c = 0; c < N; ++c) {
+            p[c] = fma(alpha, d[c], p[c]);
+            r[c] = fma(-alpha, q[c], r[c]);
+        }
+        ++k;
+        rk = (double)sqrtl(sum_planes(L, r, 1));
+        if (hist) hist[k] = rk;
+        if (!isfinite(rk)) { status = MGO_EDIVERGED; break; }
+        if (rk <= rtol * r0) { status = MGO_OK; break; }
+        if (k == max_iter) break;
+        memset(z, 0, N * sizeof(double));
+        vcycle_sym(s, 0, z, r);
+        const double rz_new = (double)dot_planes(L, r, z);
+        const double beta = rz_new / rz;
+        rz = rz_new;
+#pragma omp parallel for schedule(static)
+        for (size_t c = 0; c < N; ++c) d[c] = fma(beta, d[c], z[c]);
+    }
+    free(r); free(z); free(d); free(q);
+    if (status == MGO_EDIVERGED) { if (iters_out) *iters_out = k; return status; }
+    {
+        double mean = (double)(sum_planes(L, p, 0) / (long double)N);
+        for (size_t c = 0; c < N; ++c) p[c] = p[c] - mean;
+    }
+    if (iters_out) *iters_out = k;
+    if (relres_out) *relres_out = r0 > 0.0 ? rk / r0 : 0.0;
+    return status;
+}
+
 /* ------------------------------------------------- projection steps (S8(f) rank 2) */
 /* The two steps either side of the pressure solve in the projection method implied by
  * P:33-36 (eq. 1-2) and stated in BJ:north_star: the right-hand side div(u*)/dt from the

@@ -57,6 +57,15 @@ int  mgo_residual(mgo_solver *s, const double *rhs, const double *p, double *r_o
 int  mgo_solve(mgo_solver *s, const double *rhs, double *p, double rtol, int max_cycles,
                int *cycles_out, double *relres_out, double *hist_or_null);
 
+/* ---- MG-preconditioned CG (R22 and C12-C14 are stated in mgo.c).
+ * Needs nu1 == nu2 (MGO_EINVAL otherwise).  hist[k] = ||r_k||_2 of the recurrence residual. */
+int  mgo_solve_pcg(mgo_solver *s, const double *rhs, double *p, double rtol, int max_iter,
+                   int *iters_out, double *relres_out, double *hist_or_null);
+/* z = M r: one SYMMETRIC cycle from z = 0 (black->red post-smoothing, restriction (1/8) P^T) */
+int  mgo_precondition(mgo_solver *s, const double *r, double *z);
+/* fc = (1/8) P^T r; r on `level`, fc on level+1 */
+int  mgo_restrict_adj(const mgo_solver *s, int level, const double *r, double *fc);
+
 /* ---- projection steps either side of the solve (staggering and the
  * expression trees C10, C11 are stated in mgo.c) ----
  * f = div(u*)/dt from the staggered velocity (u,v,w on the minus faces of each cell) */

@@ -77,6 +77,9 @@ def lib():
         L.mgo_residual_level.argtypes = [vp, C.c_int, dp, dp, dp]
         L.mgo_restrict.argtypes = [vp, C.c_int, dp, dp]
         L.mgo_prolong_add.argtypes = [vp, C.c_int, dp, dp]
+        L.mgo_solve_pcg.argtypes = [vp, dp, dp, C.c_double, C.c_int, ip, dp, dp]
+        L.mgo_precondition.argtypes = [vp, dp, dp]
+        L.mgo_restrict_adj.argtypes = [vp, C.c_int, dp, dp]
         L.mgo_project_rhs.argtypes = [vp, dp, dp, dp, C.c_double, dp]
         L.mgo_project_correct.argtypes = [vp, dp, C.c_double, dp, dp, dp]
         L.mgo_threads.restype = C.c_int
@@ -178,6 +181,29 @@ class Oracle:
         if st < 0:
             raise OracleError(st)
         return st, cyc.value, rel.value, hist[: cyc.value + 1].copy()
+
+    # ---- MG-preconditioned CG
+    def solve_pcg(self, rhs, p, rtol, max_iter):
+        """Returns (status, iterations, relres, hist[0..iterations]); p updated in place."""
+        assert p.flags["C_CONTIGUOUS"] and p.dtype == np.float64 and p.shape == self.shape
+        it = C.c_int()
+        rel = C.c_double()
+        hist = np.zeros(max_iter + 1)
+        st = lib().mgo_solve_pcg(self._h, _dp(self._arr(rhs)), _dp(p), rtol, max_iter,
+                                 C.byref(it), C.byref(rel), _dp(hist))
+        if st < 0:
+            raise OracleError(st)
+        return st, it.value, rel.value, hist[: it.value + 1].copy()
+
+    def precondition(self, r):
+        z = np.empty(self.shape)
+        _chk(lib().mgo_precondition(self._h, _dp(self._arr(r)), _dp(z)))
+        return z
+
+    def restrict_adj(self, r, level=0):
+        fc = np.empty(self.level_shape(level + 1))
+        _chk(lib().mgo_restrict_adj(self._h, level, _dp(self._arr(r, level)), _dp(fc)))
+        return fc
 
     # ---- projection steps
     def project_rhs(self, u, v, w, dt):
