@@ -41,7 +41,7 @@ UNIT = "Gcell-updates/s"
 # algorithmic HBM bytes: level-0 sweep pass 32 B/cell
 # (p read+write, f, a); coarse-level pass 48 B/cell; whole V(3,3) cycle per fine cell:
 B_SWEEP_L0 = 32.0
-NCU_SWEEP_TRAFFIC_512 = 3.826e9 + 1.050e9     # bytes per launch (algorithmic: 4.295e9)
+NCU_SWEEP_TRAFFIC_512 = 3.633e9 + 1.050e9     # bytes per launch (algorithmic: 4.295e9)
 
 
 def b_sched_per_fine_cell(nu1, nu2):

@@ -43,7 +43,8 @@ constexpr int S3_NSLOT = 6;
 #ifndef S3_BAR2
 #define S3_BAR2 1
 #endif
-constexpr int S3_FPF = 4;                 // L2 prefetch distance of the f stream (planes beyond t+1)
+constexpr int S3_FAHEAD = 3;              // f is loaded this many steps before its first use
+constexpr int S3_FPF = 1;                 // L2 prefetch distance of the f stream beyond that load (measured: 1 < 2 < 4 < none)
 #ifndef S3_NST_
 #define S3_NST_ 3
 #endif
@@ -207,7 +208,7 @@ __device__ __forceinline__ void s3_body(const S3Args &A, unsigned smem_base)
     // step; the store of plane t-2 is seven planes behind it (is_out threads load and store
     // the same pair)
     size_t roff = col_bytes;
-    const size_t back_store = (size_t)(S3_NST + 4) * plane_bytes, back_f = (size_t)S3_NST * plane_bytes;
+    const size_t back_store = (size_t)(S3_NST + 4) * plane_bytes, back_f = (size_t)(S3_NST + 2 - S3_FAHEAD) * plane_bytes;
     // move a landed plane from staging slot SLOT into ring entry R and publish it to exchange slot R
     auto take = [&](auto Rc, auto Sc, unsigned sign) __attribute__((always_inline)) {
         constexpr int R = decltype(Rc)::value;
@@ -284,9 +285,13 @@ __device__ __forceinline__ void s3_body(const S3Args &A, unsigned smem_base)
     const int t0 = kz0 - 1, t_end = kz1 + 1;
     // ---- prologue: planes t0-1, t0, t0+1 -> ring entries 5, 0, 1; plane t0+2 in flight
     // (plane k uses staging slot (k - t0) mod S3_NST)
+    static_assert(S3_FAHEAD == 3, "the prologue loads f of exactly three planes");
     static_assert(S3_NST == 3 || S3_NST == 6, "staging depth must divide the unroll factor");
     issue(S3Int<S3_NST - 1>{}, t0 - 1); issue(S3Int<0>{}, t0); issue(S3Int<1>{}, t0 + 1);
-    if (S3_FDIRECT) { load_f(S3Int<0>{}, zoff(t0)); load_f(S3Int<1>{}, zoff(t0 + 1)); }
+    if (S3_FDIRECT) {
+        load_f(S3Int<0>{}, zoff(t0)); load_f(S3Int<1>{}, zoff(t0 + 1));
+        load_f(S3Int<2>{}, zoff(min(t0 + 2, kz1 + 1)));
+    }
     s3_cp_async_wait<0>();
     take(S3Int<5>{}, S3Int<S3_NST - 1>{}, zsign(t0 - 1));
     take(S3Int<0>{}, S3Int<0>{}, zsign(t0));
@@ -314,13 +319,14 @@ __device__ __forceinline__ void s3_body(const S3Args &A, unsigned smem_base)
         const int kb = t - 2;
         const int kt = STEADY ? t : s3_zmap(t, L.nz, L.bcz, sg_t);
         const int kbs = STEADY ? kb : s3_zmap(kb, L.nz, L.bcz, sg_b);
-        // f of plane t+2 -> ring (first used two steps later)
+        // f of plane t+3 -> ring, three steps before its first use (the entry it overwrites, plane
+        // t-3, was last read by the black update of step t-1); measured 2 steps: 1.04 ms, 3: 0.96 ms
         if (!S3_FDIRECT) {
         } else if (STEADY) {
-            load_f(S3Int<(U + 2) % 6>{}, roff - back_f);
+            load_f(S3Int<(U + S3_FAHEAD) % 6>{}, roff - back_f);
             s3_prefetch_l2(base_f + (roff - back_f) + S3_FPF * plane_bytes);
         } else {
-            load_f(S3Int<(U + 2) % 6>{}, zoff(min(t + 2, kz1 + 1)));
+            load_f(S3Int<(U + S3_FAHEAD) % 6>{}, zoff(min(t + S3_FAHEAD, kz1 + 1)));
         }
         // Ring-2 rows (the first and the last warp) only move data.  Everywhere else both
         // updates are evaluated unconditionally (two independent chains interleave); only
