@@ -284,3 +284,23 @@ def test_full_size_config5_bit_exact(mgmod):
     if host_gb < 100 or dev_gb < 100:
         pytest.skip(f"needs >= 100 GB host and device memory (have {host_gb:.0f} / {dev_gb:.0f})")
     _full_size_cycles(mgmod, 5, 1)
+
+
+def test_streaming_sweep_is_reproducible_under_repetition(mgmod, uniform):
+    """The streaming sweep synchronises its rows with one barrier every second step and reuses
+    its exchange and staging slots cyclically; a missing ordering would show up as run-to-run
+    differences.  40 repetitions of two sweeps on the same input (several x / y tiles and
+    z-chunks, a Neumann wall) must all give the oracle's bits."""
+    n, bc = (136, 72, 96), (P, N, P)
+    h = 1.0 / n[0]
+    shp = (n[2], n[1], n[0])
+    rho = random_rho(uniform, 9, shp)
+    o, g = pair(mgmod, n, h, bc, rho=rho)
+    f, p0 = uniform(10, shp), uniform(11, shp)
+    po = p0.copy()
+    o.sweep(f, po, 0); o.sweep(f, po, 0)
+    fd = dev(f)
+    for rep in range(40):
+        pg = dev(p0)
+        g.level_smooth(0, 2, fd, pg)
+        assert np.array_equal(po, host(pg)), f"repetition {rep}"
