@@ -415,22 +415,20 @@ inline int s3_zchunk(int nx, int ny, int nz, int num_sms)
 {
     // Long z-chunks amortise the four halo planes and the prologue of a CTA (512^3: 1.14 ms
     // per sweep with 64-plane chunks, 1.05 ms with 172), but the launch must still fill the
-    // machine in whole waves (one CTA per SM): among the chunk counts that give at least
-    // six waves' worth of CTAs (or as many as 16-plane chunks allow), take the one whose last
-    // wave is fullest.
+    // machine in whole waves (one CTA per SM): over all chunk counts (chunks of at least 16
+    // planes) take the one that maximises (filled share of the waves) x (output planes per
+    // step): 512^3 -> 3 chunks of 172, 256^3 -> 4 of 64, 1024^3 -> 2 of 512.
     const int tiles = ((nx + S3_OX - 1) / S3_OX) * ((ny + S3_OY - 1) / S3_OY);
     const int max_chunks = nz / 16 > 0 ? nz / 16 : 1;
-    int c_min = (6 * num_sms + tiles - 1) / tiles;
-    if (c_min < 1) c_min = 1;
-    if (c_min > max_chunks) c_min = max_chunks;
-    int best_c = c_min;
+    int best_c = 1;
     double best_eff = -1.0;
-    for (int c = c_min; c <= c_min + 3 && c <= max_chunks; ++c) {
+    for (int c = 1; c <= max_chunks; ++c) {
         int zc = ((nz + c - 1) / c + 1) & ~1;
         const int ctas = tiles * ((nz + zc - 1) / zc);
         const int waves = (ctas + num_sms - 1) / num_sms;
+        // fraction of SM-time slots that hold a CTA x fraction of a CTA's steps that are output planes
         const double eff = (double)ctas / ((double)waves * num_sms) * (double)zc / (double)(zc + 6);
-        if (eff > best_eff) { best_eff = eff; best_c = c; }
+        if (eff > best_eff + 1e-12) { best_eff = eff; best_c = c; }
     }
     int zc = ((nz + best_c - 1) / best_c + 1) & ~1;   // even: the colour of a component must not depend on the chunk
     if (zc > nz) zc = nz;
