@@ -165,6 +165,22 @@ def run_reference(args, w, wname):
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
+    if args.full_solve:
+        # the oracle's whole solve (time-to-rtol, cycle count), once
+        from oracle.mgo import Oracle
+        o = Oracle(w.n, w.h, w.bc, w.nu1, w.nu2)
+        o.set_density(w.rho)
+        p = np.zeros(o.shape)
+        t0 = time.perf_counter()
+        st, cyc, rel, _ = o.solve(w.rhs, p, w.rtol, 60)
+        line["full_solve"] = {"seconds": time.perf_counter() - t0, "cycles": cyc, "relres": rel, "status": st}
+        o.close()
+    try:
+        import platform
+        cpu = [l.split(":", 1)[1].strip() for l in open("/proc/cpuinfo") if l.startswith("model name")]
+        line["host"] = {"nproc": os.cpu_count(), "cpu": cpu[0] if cpu else platform.processor()}
+    except OSError:
+        pass
     print(json.dumps(line))
 
 
@@ -438,6 +454,8 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="config4", help="config<k>[@n], k = 1..5 (BASELINE.json configs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--full-solve", action="store_true",
+                    help="reference arm only: also time the oracle's whole solve once")
     ap.add_argument("--sequence", type=int, default=0,
                     help="also run a K-step falling-drop sequence (set_density + warm-started solve per step)")
     ap.add_argument("--no-projection", dest="projection", action="store_false",
