@@ -1,31 +1,42 @@
-// mg_sweep_kernels.cuh -- streaming red-black Gauss-Seidel sweep, generation 3.
+// mg_sweep_kernels.cuh -- the level-0 smoother: one full red-black Gauss-Seidel sweep (red
+// half-sweep, then black, R9) in ONE streaming pass, read from p_in and written to p_out:
+// 32 B per cell of compulsory HBM traffic (p in, p out, f, a).
 //
-// One launch = one full sweep (red half-sweep, then black, R9) read from p_in and written
-// to p_out: 32 B per cell of compulsory HBM traffic on level 0 (p in, p out, f, a).
+// Geometry.  A CTA owns an (x,y) tile of 64 x S3_TY cells including a halo of 2 and marches
+// through a z-chunk.  A warp is one tile row; thread (lx,ly) owns the column of the aligned
+// x-pair (2lx, 2lx+1) of row ly and keeps the z-window of its two cells (planes t+3 .. t-3 of
+// p, a, f) in a compile-time-indexed register ring (6-fold unrolled step).  At step t it
+// updates its red cell of plane t and its black cell of plane t-2; ring 1 of the tile
+// recomputes the red values the neighbouring CTA also computes (same expression tree, same
+// inputs, same bits), so exact global red->black semantics are kept; rows 0 and S3_TY-1
+// (ring 2) only move data.
 //
-// Geometry (as generation 2, mg_stream_kernels.cuh): a CTA owns an (x,y) tile of
-// 64 x S3_TY cells including a halo of 2 and marches through a z-chunk.  Thread (lx,ly)
-// owns the column of the aligned x-pair (2lx, 2lx+1) of tile row ly and keeps the
-// z-window of its two cells (planes t+2 .. t-3 of p, a, f) in a compile-time-indexed
-// register ring.  At step t it updates its red cell of plane t and its black cell of
-// plane t-2; ring 1 of the tile recomputes the red values the neighbouring CTA also
-// computes (same expression tree, same inputs, same bits), so exact global red->black
-// semantics are kept.
+// Data movement (history and measurements: profiles/r1b_sweep.md, r1d_cycle.md):
+//   * p and a: cp.async (16 B, .ca) of the thread's own pair into private staging slots, three
+//     planes in flight; a thread only reads back what it copied itself, so staging needs no
+//     barrier, only cp.async.wait_group;
+//   * f never needs to be shared: LDG.128 straight into the ring three steps before its first
+//     use, with an L2 prefetch one plane further;
+//   * exchange planes in shared memory hold (p, a) as one 16-byte entry per cell, split by
+//     colour class: one conflict-free LDS.128 fetches a neighbour's value AND its coefficient
+//     (6 neighbour reads + 2 staging reads + 3 stores, all 128-bit, per thread and step);
+//   * six exchange slots = the ring length, so every shared-memory address of the unrolled
+//     loop is a per-thread base plus a compile-time offset;
+//   * everything a step writes to shared memory is first read two steps later and every slot
+//     it overwrites was last read two steps earlier: ONE barrier every SECOND step;
+//   * steady-state steps (all touched planes inside the domain and the chunk) carry no index
+//     mapping and no range tests; the z-chunk length is chosen so that the CTAs fill whole
+//     waves of the machine (s3_zchunk).
 //
-// What changed against generation 2 (profiles/r1a_baseline.md: 190 warp instructions
-// per plane step, ~26 shared-memory operations per thread per step, issue-bound):
-//   * global loads go straight into registers (one LDG.128 per array per plane per
-//     thread, issued one full step ahead; an L2 prefetch runs S3_PF planes ahead) --
-//     no staging buffers, no collect pass;
-//   * the exchange planes in shared memory hold (p, a) interleaved as one 16-byte entry
-//     per cell, de-interleaved by colour class: one conflict-free LDS.128 fetches a
-//     neighbour's value AND its coefficient (6 LDS.128 + 3 STS.128 per thread per step);
-//   * six exchange slots = the register ring length, so every shared-memory address in
-//     the 6-fold unrolled loop is a per-thread base plus a compile-time offset, and a
-//     new plane can be published before the step's single barrier;
-//   * a Neumann ghost pair is reversed by swapping its two publish addresses (free)
-//     and its sign flip (a_ghost = -a_mirror, so that a wall face is exactly +0.0, C2)
-//     is one XOR with a per-thread mask.
+// Boundaries.  Indices outside the domain are wrapped (periodic) or mirrored (Neumann) at
+// load time.  A Neumann ghost cell carries a = -a(mirror), so the canonical face
+// beta = a_c + a_nb evaluates to exactly +0.0 on a wall face (C2) with no wall logic in the
+// update (one XOR with a per-thread sign mask); ghost cells themselves are never updated.  A
+// mirrored x-pair arrives reversed: its two publish addresses are swapped (free).
+//
+// Only the CELL = true instance (level 0) is built.  The stored-face branch (CELL = false) of
+// the template lost against the half-sweep launches on every level size (profiles/r1d_cycle.md)
+// and is not instantiated; the cycle uses k_smooth_half on levels >= 1.
 #pragma once
 #include "mg_common.cuh"
 
@@ -458,7 +469,8 @@ inline int launch_sweep3(Lv L, bool cell, const double *f, const double *pin, do
 {
     S3Args a;
     a.L = L; a.f = f; a.pin = pin; a.pout = pout; a.zchunk = 0;
-    return cell ? s3_launch<true>(a, num_sms, st) : s3_launch<false>(a, num_sms, st);
+    if (!cell) return -1;                 // stored-face levels use the half-sweep kernels
+    return s3_launch<true>(a, num_sms, st);
 }
 
 } // namespace mg
