@@ -28,9 +28,13 @@
  * modes, symmetry / zero row+column sums, the layered-medium prefix-sum solution,
  * second-order convergence on a manufactured solution, a dense direct solve at 8^3,
  * smoother and transfer invariants, config 1's known solution.
- * PARITY UNPINNED (conventions with no external pin): R8 (4-face coarse
- * rule), R13 (coarsest sweep count), R11 (8-child mean among the "full-weighting"
- * readings), R18 (sphere position in the input recipe).
+ * The coarse-face rule C3 is pinned value by value against numpy slices of the finer level's
+ * faces on a fully 3-D random density (test_coarse_faces_brute_force_3d); the coarsest-level
+ * sweep count against a one-level hierarchy (test_coarsest_level_runs_exactly_coarse_sweeps_sweeps).
+ * PARITY UNPINNED (CHOICES among readings on which the paper is silent, not functions: what
+ * the code computes under each choice is pinned): that R8 is the 4-face mean,
+ * that R13's default is 32 sweeps, that R11 is the 8-child mean among the "full-weighting"
+ * readings, R18 (sphere position in the input recipe).
  *
  * All pointers are HOST pointers to dense fp64 arrays, idx = i + nx*(j + ny*k).
  */

@@ -364,6 +364,62 @@ def test_coarse_faces_invariants(uniform):
     assert np.allclose(bz1[:, 3, 3], bz0[0::2, 3, 3], rtol=1e-15)   # even child's minus face
 
 
+@pytest.mark.parametrize("bc", [(P, P, P), (P, N, N), (N, N, N)])
+def test_coarse_faces_brute_force_3d(bc, uniform):
+    """Pins mgo_set_density's coarse levels: with a fully 3-D
+    random density every face of level l >= 1 must be the mean of the FOUR level l-1 faces of the
+    same direction that lie on it, i.e. the minus faces of the even child across the face and
+    of its three neighbours in the two tangential directions, written out as numpy slices of
+    faces(l-1) in (k, j, i) order.  Catches: taking the odd child's face, averaging over the
+    wrong pair of directions, dropping one of the four faces (each changes the value when
+    the density varies in all three directions)."""
+    n = (32, 16, 16)                      # nx != ny: catches a swapped axis as well
+    o = Oracle(n, 1.0 / 16, bc)
+    o.set_density(np.exp(uniform(83, o.shape, 0.0, 6.0)))
+    assert o.num_levels >= 3
+    for lvl in range(1, o.num_levels):
+        fx, fy, fz = o.faces(lvl - 1)
+        bx, by, bz = o.faces(lvl)
+        # x-face of coarse cell (I,J,K): fine x-minus faces at i = 2I, j in {2J,2J+1}, k in {2K,2K+1}
+        ex = 0.25 * ((fx[0::2, 0::2, 0::2] + fx[0::2, 1::2, 0::2]) + (fx[1::2, 0::2, 0::2] + fx[1::2, 1::2, 0::2]))
+        # y-face: fine y-minus faces at j = 2J, i in {2I,2I+1}, k in {2K,2K+1}
+        ey = 0.25 * ((fy[0::2, 0::2, 0::2] + fy[0::2, 0::2, 1::2]) + (fy[1::2, 0::2, 0::2] + fy[1::2, 0::2, 1::2]))
+        # z-face: fine z-minus faces at k = 2K, i in {2I,2I+1}, j in {2J,2J+1}
+        ez = 0.25 * ((fz[0::2, 0::2, 0::2] + fz[0::2, 0::2, 1::2]) + (fz[0::2, 1::2, 0::2] + fz[0::2, 1::2, 1::2]))
+        for got, exp in ((bx, ex), (by, ey), (bz, ez)):
+            assert got.shape == exp.shape
+            assert np.all(np.abs(got - exp) <= np.spacing(np.abs(exp)))     # 1 ulp
+        # the random field really separates the candidates (odd child / wrong pair / 3 of 4)
+        odd = 0.25 * ((fx[0::2, 0::2, 1::2] + fx[0::2, 1::2, 1::2]) + (fx[1::2, 0::2, 1::2] + fx[1::2, 1::2, 1::2]))
+        assert np.abs(odd - ex).max() > 1e-3 * np.abs(ex).max()
+        # Neumann axes keep their wall face exactly zero on every level
+        if bc[0] == N: assert np.all(bx[:, :, 0] == 0.0)
+        if bc[1] == N: assert np.all(by[:, 0, :] == 0.0)
+        if bc[2] == N: assert np.all(bz[0] == 0.0)
+
+
+def test_coarsest_level_runs_exactly_coarse_sweeps_sweeps(uniform):
+    """Pins R13's count in vcycle(): on a one-level hierarchy (6^3 cannot be halved, R7) a cycle
+    is nothing but `coarse_sweeps` red-black sweeps from the incoming p, each of which is the
+    pinned smooth_half(0) then smooth_half(1).  Catches a wrong count (e.g. coarse_sweeps/8) and
+    a coarsest solve that restarts from zero."""
+    o = Oracle((6, 6, 6), 1.0 / 6, (P, N, P), 2, 2, 5)
+    assert o.num_levels == 1
+    o.set_density(np.exp(uniform(85, o.shape, 0.0, 3.0)))
+    f = uniform(86, o.shape)
+    f -= f.mean()
+    p0 = uniform(87, o.shape)
+    p = p0.copy()
+    o.vcycle(f, p)
+    q = p0.copy()
+    for it in range(5):
+        o.smooth_half(0, f, q)
+        o.smooth_half(1, f, q)
+        if it == 3:
+            assert not np.array_equal(p, q)          # four sweeps are not enough
+    assert np.array_equal(p, q)
+
+
 # --------------------------------------------------------------------------- #
 # 9. end to end on config 1 (known solution), API behaviour, thread independence
 # --------------------------------------------------------------------------- #
