@@ -28,7 +28,8 @@
  * Conventions.  All functions return an int status: MG_OK (0), MG_NOT_CONVERGED (1) or
  * a negative error.  No exception crosses the ABI.  A handle is not thread-safe.
  * Pointers named *_dev are DEVICE pointers (cudaMalloc / torch tensor .data_ptr()) to
- * fp64 data on the device that was current at mg_create; *_host are HOST pointers.
+ * fp64 data on the device that was current at mg_create, aligned to 16 bytes (the kernels
+ * move cell pairs; a misaligned pointer is rejected with MG_EINVAL); *_host are HOST pointers.
  * The library never frees or keeps caller buffers beyond what each call states.  Work
  * is enqueued on the handle's stream (mg_set_stream); calls that return a host value
  * synchronise that stream, the others are asynchronous.

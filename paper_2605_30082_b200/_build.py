@@ -23,7 +23,7 @@ NVCC_FLAGS = [
     "-lineinfo", "-O3", "-std=c++17",
     "-fmad=false",                 # no implicit contraction: all fma are explicit
     "-Xcompiler", "-fPIC", "-shared",
-] + os.environ.get("MG_NVCC_EXTRA", "").split()     # e.g. -DS3_BAR2=0 for kernel experiments
+]
 
 
 def sources():
@@ -51,15 +51,24 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     if out.exists() and not force:
         return out
     LIBDIR.mkdir(exist_ok=True)
-    for old in LIBDIR.glob("libmg-*.so"):
-        old.unlink()
-    tmp = out.with_suffix(f".tmp{os.getpid()}")
-    cmd = [nvcc(), *NVCC_FLAGS, "-o", str(tmp), str(CSRC / "mg.cu")]
-    if verbose:
-        cmd.insert(1, "-Xptxas=-v")
-        print(" ".join(cmd))
-    subprocess.run(cmd, check=True, cwd=CSRC)
-    os.replace(tmp, out)
+    import fcntl
+
+    # several ranks may import at once (torchrun): one builds, the others wait for the lock and
+    # find the library; stale hashes are removed only after the new file is in place
+    with open(LIBDIR / ".build.lock", "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        if out.exists() and not force:
+            return out
+        tmp = out.with_suffix(f".tmp{os.getpid()}")
+        cmd = [nvcc(), *NVCC_FLAGS, "-o", str(tmp), str(CSRC / "mg.cu")]
+        if verbose:
+            cmd.insert(1, "-Xptxas=-v")
+            print(" ".join(cmd))
+        subprocess.run(cmd, check=True, cwd=CSRC)
+        os.replace(tmp, out)
+        for old in LIBDIR.glob("libmg-*.so"):
+            if old != out:
+                old.unlink()
     return out
 
 

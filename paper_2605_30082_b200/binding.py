@@ -93,6 +93,7 @@ def _ptr(t, shape=None):
         "expected a contiguous CUDA float64 tensor"
     if shape is not None:
         assert tuple(t.shape) == tuple(shape), (tuple(t.shape), tuple(shape))
+    assert t.data_ptr() % 16 == 0, "device arrays must be 16-byte aligned (include/mg.h)"
     return t.data_ptr()
 
 
@@ -101,7 +102,8 @@ class Multigrid:
     1 Neumann).  Device storage comes from a torch tensor (mg_create_in); the stream is
     torch's current stream at construction unless ``stream`` is given."""
 
-    def __init__(self, n, h, bc, nu1=2, nu2=2, coarse_sweeps=32, stream=None, device="cuda:0"):
+    def __init__(self, n, h, bc, nu1=2, nu2=2, coarse_sweeps=32, stream=None, device="cuda:0",
+                 own_workspace=False):
         import torch
 
         nx, ny, nz = (n, n, n) if isinstance(n, int) else n
@@ -114,10 +116,14 @@ class Multigrid:
         if need == 0:
             raise MgError(MG_EINVAL)
         with torch.cuda.device(self.device):
-            self._ws = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
-            base = (self._ws.data_ptr() + 255) // 256 * 256
             bca = (C.c_int * 3)(*[int(b) for b in bc])
-            _chk(L.mg_create_in(*self.n, float(h), bca, base, need, C.byref(self._h)))
+            if own_workspace:           # mg_create: the library allocates with cudaMalloc
+                self._ws = None
+                _chk(L.mg_create(*self.n, float(h), bca, C.byref(self._h)))
+            else:
+                self._ws = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
+                base = (self._ws.data_ptr() + 255) // 256 * 256
+                _chk(L.mg_create_in(*self.n, float(h), bca, base, need, C.byref(self._h)))
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             _chk(L.mg_set_stream(self._h, self.stream.cuda_stream))
         _chk(L.mg_set_cycle(self._h, nu1, nu2, coarse_sweeps))
@@ -173,6 +179,11 @@ class Multigrid:
         _chk(lib().mg_residual(self._h, _ptr(rhs, self.shape), _ptr(p, self.shape),
                                _ptr(r, self.shape), C.byref(nrm)))
         return nrm.value
+
+    def residual_field(self, rhs, p, r):
+        """r = rhs - A p only (no norm, asynchronous)."""
+        _chk(lib().mg_residual(self._h, _ptr(rhs, self.shape), _ptr(p, self.shape), _ptr(r, self.shape), None))
+        return r
 
     def solve(self, rhs, p, rtol, max_cycles):
         """Returns (status, cycles, relres, hist[0..cycles]); p updated in place."""

@@ -224,18 +224,19 @@ __global__ void __launch_bounds__(kCoarseThreads, 1) k_coarse_cta(CoarseArgs A)
     }
 }
 
+// opt-in to the dynamic shared memory the kernel needs; per device, called from mg_create
+inline int coarse_cta_prepare_device()
+{
+    return cudaFuncSetAttribute(k_coarse_cta, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)kCoarseSmemMax) == cudaSuccess ? 0 : -1;
+}
+
 inline int launch_coarse_cta(const CoarseArgs &a, cudaStream_t st)
 {
-    static size_t attr_bytes = 0;
     int n[kCoarseMaxLevels][3];
     for (int q = 0; q < a.nlev; ++q) { n[q][0] = a.n[q][0]; n[q][1] = a.n[q][1]; n[q][2] = a.n[q][2]; }
     const size_t bytes = coarse_cta_bytes(n, a.nlev);
-    if (bytes > attr_bytes) {
-        if (cudaFuncSetAttribute(k_coarse_cta, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) !=
-            cudaSuccess)
-            return -1;
-        attr_bytes = bytes;
-    }
+    if (bytes > kCoarseSmemMax) return -1;
     k_coarse_cta<<<1, kCoarseThreads, bytes, st>>>(a);
     return 0;
 }

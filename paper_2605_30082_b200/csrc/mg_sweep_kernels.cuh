@@ -446,16 +446,17 @@ inline int s3_zchunk(int nx, int ny, int nz, int num_sms)
     return zc;
 }
 
+// opt-in to the dynamic shared memory of k_sweep3; per device, called from mg_create
+inline int sweep3_prepare_device()
+{
+    return cudaFuncSetAttribute(k_sweep3<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)S3_SMEM_BYTES) == cudaSuccess ? 0 : -1;
+}
+
 template <bool CELL>
 inline int s3_launch(const S3Args &a, int num_sms, cudaStream_t st)
 {
-    static bool attr_done = false;
     auto kern = k_sweep3<CELL>;
-    if (!attr_done) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S3_SMEM_BYTES) != cudaSuccess)
-            return -1;
-        attr_done = true;
-    }
     S3Args b = a;
     b.zchunk = s3_zchunk(a.L.nx, a.L.ny, a.L.nz, num_sms);
     dim3 grid((a.L.nx + S3_OX - 1) / S3_OX, (a.L.ny + S3_OY - 1) / S3_OY, (a.L.nz + b.zchunk - 1) / b.zchunk);

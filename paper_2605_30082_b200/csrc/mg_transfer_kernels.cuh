@@ -280,7 +280,7 @@ __global__ void __launch_bounds__(128) k_prolong_stream(PrArgs A)
                 v[s] = lerp(yc, yf);
             }
             const size_t c = (size_t)(2 * I) + (size_t)A.nx * (size_t)(2 * J + t) + fplane * (size_t)(2 * K + u);
-            const double2 pi = __ldg(reinterpret_cast<const double2 *>(A.pin + c));
+            const double2 pi = *reinterpret_cast<const double2 *>(A.pin + c);   // plain load: p_out may alias p_in
             double2 po;
             po.x = __dadd_rn(pi.x, v[0]);
             po.y = __dadd_rn(pi.y, v[1]);

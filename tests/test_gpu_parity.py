@@ -188,6 +188,82 @@ def test_solve_host_buffers(mgmod):
 
 
 # --------------------------------------------------------------------------- #
+# paths of the boundary that the tests above do not reach
+# --------------------------------------------------------------------------- #
+@pytest.mark.parametrize("n,bc", [((72, 40, 36), (P, N, N)), ((64, 64, 64), (P, P, N))])
+def test_residual_field_and_norm(mgmod, uniform, n, bc):
+    """mg_residual with r_dev: the field alone (norm2_host NULL) and field + norm in one call
+    (DESIGN §3 C6, R15): r bit-exact, the norm within 1e-10."""
+    shp = (n[2], n[1], n[0])
+    o, g = pair(mgmod, n, 1.0 / n[0], bc, rho=random_rho(uniform, 41, shp))
+    f, p = uniform(42, shp), uniform(43, shp)
+    nrm_o, r_o = o.residual(f, p, want_field=True)
+    fd, pd = dev(f), dev(p)
+    r1 = torch.full(shp, np.nan, dtype=torch.float64, device="cuda:0")
+    g.residual_field(fd, pd, r1)
+    assert np.array_equal(r_o, host(r1))
+    r2 = torch.full(shp, np.nan, dtype=torch.float64, device="cuda:0")
+    nrm_g = g.residual(fd, pd, r2)
+    assert np.array_equal(r_o, host(r2))
+    assert nrm_g == pytest.approx(nrm_o, rel=NORM_RTOL)
+    assert g.residual(fd, pd) == pytest.approx(nrm_o, rel=NORM_RTOL)
+
+
+def test_warm_started_solve_after_density_replacement(mgmod):
+    """The time-sequence path (bench.py --sequence): solve, replace the
+    density, solve again from the previous solution.  Same cycle counts, norms 1e-10, p 1e-9."""
+    from workloads import sequence_density
+    w = make_workload(3, 64)
+    o, g = pair(mgmod, w.n, w.h, w.bc, nu=(w.nu1, w.nu2))
+    po, pg, fd = np.zeros(o.shape), dev(np.zeros(o.shape)), dev(w.rhs)
+    for step in range(3):
+        rho = sequence_density(3, 64, step, 3)
+        o.set_density(rho)
+        g.set_density(dev(rho))
+        so, co, ro, ho = o.solve(w.rhs, po, w.rtol, 40)       # po, pg: previous step's solution
+        sg, cg, rg, hg = g.solve(fd, pg, w.rtol, 40)
+        assert (sg, cg) == (so, co), f"step {step}"
+        assert np.all(np.abs(np.array(hg) / ho - 1) <= NORM_RTOL), f"step {step}"
+        assert np.abs(host(pg) - po).max() <= P_RTOL * np.abs(po).max(), f"step {step}"
+        if step:
+            assert co < 10                                     # the warm start pays
+
+
+def test_library_owned_workspace(mgmod, uniform):
+    """mg_create (cudaMalloc workspace owned by the handle) instead of mg_create_in."""
+    n, bc = (64, 32, 48), (P, N, P)
+    shp = (n[2], n[1], n[0])
+    rho = random_rho(uniform, 44, shp)
+    o = Oracle(n, 1.0 / 64, bc, 2, 2)
+    g = mgmod.Multigrid(n, 1.0 / 64, bc, 2, 2, own_workspace=True)
+    o.set_density(rho)
+    g.set_density(dev(rho))
+    f = uniform(45, shp)
+    f -= f.mean()
+    po, pg, fd = np.zeros(shp), dev(np.zeros(shp)), dev(f)
+    for cyc in range(2):
+        o.vcycle(f, po)
+        g.vcycle(fd, pg)
+        assert np.array_equal(po, host(pg))
+    g.close()
+
+
+def test_full_solve_config3_256(mgmod):
+    """BASELINE configs[2] at its full size (256^3 drop-film, V(3,3), 1e-8): the whole solve,
+    every norm of the history and the solution, in the launch configuration bench.py times."""
+    check_solve(mgmod, make_workload(3))
+
+
+def test_misaligned_device_pointer_is_rejected(mgmod):
+    from paper_2605_30082_b200 import binding as B
+    g = mgmod.Multigrid((8, 8, 8), 0.125, (P, P, P))
+    buf = torch.zeros(8 * 8 * 8 + 1, dtype=torch.float64, device="cuda:0")
+    ok = buf[:512]
+    st = B.lib().mg_vcycle(g._h, ok.data_ptr() + 8, ok.data_ptr())
+    assert st == B.MG_EINVAL
+
+
+# --------------------------------------------------------------------------- #
 # edge cases and error behaviour of the boundary
 # --------------------------------------------------------------------------- #
 def test_error_codes_and_degenerate_inputs(mgmod, uniform):
