@@ -211,7 +211,14 @@ def test_residual_field_and_norm(mgmod, uniform, n, bc):
 
 def test_warm_started_solve_after_density_replacement(mgmod):
     """The time-sequence path (bench.py --sequence): solve, replace the
-    density, solve again from the previous solution.  Same cycle counts, norms 1e-10, p 1e-9."""
+    density, solve again from the previous solution.
+    (a) Identical inputs: each GPU solve starts from the ORACLE's previous solution, so both
+        sides see the same bits: cycle counts equal, norms 1e-10 relative, p 1e-9.
+    (b) The GPU's own chain: its starting iterate differs from the oracle's by the rounding of
+        the subtracted mean (C9 leaves the summation order free, ~1e-18 relative).  That
+        perturbation is amplified relative to the shrinking residual (SURVEY §8(c) "parity
+        hazard"), so the chain is held to SURVEY's stated fallback reading
+        |d||r_k||| <= 1e-10 ||r_0||, plus equal cycle counts and p within 1e-9."""
     from workloads import sequence_density
     w = make_workload(3, 64)
     o, g = pair(mgmod, w.n, w.h, w.bc, nu=(w.nu1, w.nu2))
@@ -220,10 +227,15 @@ def test_warm_started_solve_after_density_replacement(mgmod):
         rho = sequence_density(3, 64, step, 3)
         o.set_density(rho)
         g.set_density(dev(rho))
+        pg_same = dev(po)                                     # (a): the oracle's starting iterate
         so, co, ro, ho = o.solve(w.rhs, po, w.rtol, 40)       # po, pg: previous step's solution
-        sg, cg, rg, hg = g.solve(fd, pg, w.rtol, 40)
+        sa, ca, ra, ha = g.solve(fd, pg_same, w.rtol, 40)
+        assert (sa, ca) == (so, co), f"step {step}"
+        assert np.all(np.abs(np.array(ha) / ho - 1) <= NORM_RTOL), f"step {step}"
+        assert np.abs(host(pg_same) - po).max() <= P_RTOL * np.abs(po).max(), f"step {step}"
+        sg, cg, rg, hg = g.solve(fd, pg, w.rtol, 40)          # (b): the GPU's own chain
         assert (sg, cg) == (so, co), f"step {step}"
-        assert np.all(np.abs(np.array(hg) / ho - 1) <= NORM_RTOL), f"step {step}"
+        assert np.abs(np.array(hg) - ho).max() <= NORM_RTOL * ho[0], f"step {step}"
         assert np.abs(host(pg) - po).max() <= P_RTOL * np.abs(po).max(), f"step {step}"
         if step:
             assert co < 10                                     # the warm start pays
