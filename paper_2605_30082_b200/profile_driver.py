@@ -26,6 +26,7 @@ def main():
     ap.add_argument("--reps", type=int, default=5)
     ap.add_argument("--kernels", type=int, default=1)
     ap.add_argument("--graph", type=int, default=1)
+    ap.add_argument("--fuse", type=int, default=1)
     args = ap.parse_args()
     body = args.workload[len("config"):]
     cfg, n = (body.split("@") + [None])[:2]
@@ -35,6 +36,7 @@ def main():
         g = mgpkg.Multigrid(w.n, w.h, w.bc, w.nu1, w.nu2, stream=st)
         g.set_option(B.MG_OPT_KERNELS, args.kernels)
         g.set_option(B.MG_OPT_GRAPH, args.graph)
+        g.set_option(B.MG_OPT_SWEEP_FUSE, args.fuse)
         g.set_density(torch.from_numpy(w.rho).cuda())
         shp = g.level_shape(args.level)
         if args.level == 0:
@@ -44,7 +46,9 @@ def main():
         p = torch.zeros(shp, dtype=torch.float64, device="cuda")
 
         def run():
-            if args.step == "sweep2":
+            if args.step == "sweep4":
+                g.level_smooth(args.level, 4, f, p)
+            elif args.step == "sweep2":
                 g.level_smooth(args.level, 2, f, p)
             elif args.step == "sweep1":
                 g.level_smooth(args.level, 1, f, p)
