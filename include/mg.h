@@ -64,7 +64,10 @@ enum {
                                2 = as 1 with the cp.async register-ring sweep of round 1     */
     MG_OPT_GRAPH = 2,       /* 1 (default) = V-cycle replayed from a captured CUDA graph     */
     MG_OPT_COARSE_CTA = 3,  /* 1 (default) = levels <= 16^3 run in one persistent CTA       */
-    MG_OPT_SWEEP_FUSE = 4   /* level-0 sweeps fused per pass of the TMA kernel: 1 (default) or 2 */
+    MG_OPT_SWEEP_FUSE = 4,  /* level-0 sweeps fused per pass of the TMA kernel: 1 (default) or 2 */
+    MG_OPT_TAIL_FUSION = 5  /* 1 (default) = residual+restriction fused behind the last pre-sweep,
+                               prolongation in front of the first post-sweep and, in mg_solve,
+                               sum r^2 behind the last post-sweep (level 0); 0 = separate passes */
 };
 
 /* mg_get_stat keys */
@@ -178,6 +181,13 @@ int mg_level_residual(mg_handle *s, int level, const double *f_dev, const double
 /* fc = 8-child mean of (f - A_level p): fused residual + restriction, level -> level+1 */
 int mg_level_residual_restrict(mg_handle *s, int level, const double *f_dev,
                                const double *p_dev, double *fc_dev);
+/* `sweeps` (>= 1) sweeps in place on p, then fc = 8-child mean of (f - A_level p): the last
+ * pre-sweep of the cycle with steps A2+A3 fused behind it (level 0: one pass of the TMA kernel) */
+int mg_level_smooth_restrict(mg_handle *s, int level, int sweeps, const double *f_dev, double *p_dev,
+                             double *fc_dev);
+/* `sweeps` (>= 1) level-0 sweeps in place on p, then sqrt(sum (f - A p)^2) to *norm2_host: the
+ * last post-sweep of mg_solve's cycle with step A7 fused behind it.  Synchronises the stream. */
+int mg_level_smooth_norm(mg_handle *s, int sweeps, const double *f_dev, double *p_dev, double *norm2_host);
 /* p += trilinear prolongation of e (e on level+1, p on level) */
 int mg_level_prolong_add(mg_handle *s, int level, const double *e_dev, double *p_dev);
 

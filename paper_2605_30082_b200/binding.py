@@ -13,7 +13,7 @@ from . import _build
 MG_OK, MG_NOT_CONVERGED = 0, 1
 MG_EINVAL, MG_ENOMEM, MG_ECUDA, MG_EINCOMPATIBLE, MG_EDIVERGED = -1, -2, -3, -4, -5
 MG_BC_PERIODIC, MG_BC_NEUMANN = 0, 1
-MG_OPT_KERNELS, MG_OPT_GRAPH, MG_OPT_COARSE_CTA, MG_OPT_SWEEP_FUSE = 1, 2, 3, 4
+MG_OPT_KERNELS, MG_OPT_GRAPH, MG_OPT_COARSE_CTA, MG_OPT_SWEEP_FUSE, MG_OPT_TAIL_FUSION = 1, 2, 3, 4, 5
 MG_STAT_KERNEL_LAUNCHES, MG_STAT_WORKSPACE_BYTES, MG_STAT_LAUNCHES_PER_VCYCLE = 1, 2, 3
 
 _vp, _dp, _ip = C.c_void_p, C.c_void_p, C.POINTER(C.c_int)   # device pointers travel as integers
@@ -46,6 +46,8 @@ SIGNATURES = {
     "mg_level_residual": (C.c_int, [_vp, C.c_int, _dp, _dp, _dp]),
     "mg_level_residual_restrict": (C.c_int, [_vp, C.c_int, _dp, _dp, _dp]),
     "mg_level_prolong_add": (C.c_int, [_vp, C.c_int, _dp, _dp]),
+    "mg_level_smooth_restrict": (C.c_int, [_vp, C.c_int, C.c_int, _dp, _dp, _dp]),
+    "mg_level_smooth_norm": (C.c_int, [_vp, C.c_int, _dp, _dp, _hp]),
 }
 
 _lib = None
@@ -261,6 +263,19 @@ class Multigrid:
         shp = self.level_shape(level)
         _chk(lib().mg_level_residual_restrict(self._h, level, _ptr(f, shp), _ptr(p, shp), _ptr(fc)))
         return fc
+
+    def level_smooth_restrict(self, level, sweeps, f, p):
+        import torch
+
+        fc = torch.empty(self.level_shape(level + 1), dtype=torch.float64, device=self.device)
+        shp = self.level_shape(level)
+        _chk(lib().mg_level_smooth_restrict(self._h, level, sweeps, _ptr(f, shp), _ptr(p, shp), _ptr(fc)))
+        return fc
+
+    def level_smooth_norm(self, sweeps, f, p):
+        nrm = C.c_double()
+        _chk(lib().mg_level_smooth_norm(self._h, sweeps, _ptr(f, self.shape), _ptr(p, self.shape), C.byref(nrm)))
+        return nrm.value
 
     def level_prolong_add(self, level, e, p):
         _chk(lib().mg_level_prolong_add(self._h, level, _ptr(e, self.level_shape(level + 1)),

@@ -43,7 +43,8 @@ def pair(mgmod, n, h, bc, nu=(2, 2), rho=None, coarse_sweeps=32, **opts):
     o = Oracle(n, h, bc, nu[0], nu[1], coarse_sweeps)
     g = mgmod.Multigrid(n, h, bc, nu[0], nu[1], coarse_sweeps)
     from paper_2605_30082_b200 import binding as B
-    for key, name in ((B.MG_OPT_KERNELS, "kernels"), (B.MG_OPT_GRAPH, "graph"), (B.MG_OPT_COARSE_CTA, "coarse_cta")):
+    for key, name in ((B.MG_OPT_KERNELS, "kernels"), (B.MG_OPT_GRAPH, "graph"), (B.MG_OPT_COARSE_CTA, "coarse_cta"),
+                      (B.MG_OPT_TAIL_FUSION, "tails"), (B.MG_OPT_SWEEP_FUSE, "fuse")):
         if name in opts:
             g.set_option(key, opts[name])
     if rho is not None:
@@ -113,13 +114,76 @@ def test_steps_bit_exact(mgmod, uniform, n, bc):
 
 
 # --------------------------------------------------------------------------- #
+# fused tails of the TMA sweep kernel (SURVEY §8(a) A2+A3 behind the last pre-sweep, A7 behind
+# the last post-sweep): p and the coarse right-hand side bit-exact, norm 1e-10
+# --------------------------------------------------------------------------- #
+TAIL_SHAPES = [
+    ((64, 64, 64), (P, P, P)),
+    ((64, 64, 64), (N, N, N)),
+    ((72, 40, 36), (P, N, N)),      # ragged tiles, x periodic through a shifted last tile
+    ((136, 72, 96), (N, P, P)),     # several tiles per axis and several z-chunks
+    ((32, 32, 32), (P, P, N)),
+]
+
+
+@pytest.mark.parametrize("n,bc", TAIL_SHAPES)
+@pytest.mark.parametrize("sweeps", [1, 2, 3])
+def test_fused_restrict_tail_bit_exact(mgmod, uniform, n, bc, sweeps):
+    shp = (n[2], n[1], n[0])
+    o, g = pair(mgmod, n, 1.0 / n[0], bc, rho=random_rho(uniform, 51, shp))
+    f, p0 = uniform(52, shp), uniform(53, shp)
+    po = p0.copy()
+    for _ in range(sweeps):
+        o.sweep(f, po, 0)
+    fc_o = o.restrict(o.residual_level(f, po, 0), 0)
+    pg = dev(p0)
+    fc_g = g.level_smooth_restrict(0, sweeps, dev(f), pg)
+    assert np.array_equal(po, host(pg))
+    assert np.array_equal(fc_o, host(fc_g))
+
+
+@pytest.mark.parametrize("n,bc", TAIL_SHAPES)
+@pytest.mark.parametrize("sweeps", [1, 2])
+def test_fused_norm_tail(mgmod, uniform, n, bc, sweeps):
+    shp = (n[2], n[1], n[0])
+    o, g = pair(mgmod, n, 1.0 / n[0], bc, rho=random_rho(uniform, 54, shp))
+    f, p0 = uniform(55, shp), uniform(56, shp)
+    po = p0.copy()
+    for _ in range(sweeps):
+        o.sweep(f, po, 0)
+    pg = dev(p0)
+    nrm = g.level_smooth_norm(sweeps, dev(f), pg)
+    assert np.array_equal(po, host(pg))
+    assert nrm == pytest.approx(o.residual(f, po), rel=NORM_RTOL)
+
+
+@pytest.mark.parametrize("sweeps", [2, 4, 5])
+def test_two_sweeps_fused_per_pass_bit_exact(mgmod, uniform, sweeps):
+    """MG_OPT_SWEEP_FUSE = 2: temporal blocking, two red-black sweeps per pass of k_rbt<2>."""
+    from paper_2605_30082_b200 import binding as B
+    n, bc = (136, 72, 96), (P, N, P)
+    shp = (n[2], n[1], n[0])
+    o, g = pair(mgmod, n, 1.0 / n[0], bc, rho=random_rho(uniform, 57, shp))
+    g.set_option(B.MG_OPT_SWEEP_FUSE, 2)
+    f, p0 = uniform(58, shp), uniform(59, shp)
+    po = p0.copy()
+    for _ in range(sweeps):
+        o.sweep(f, po, 0)
+    pg = dev(p0)
+    g.level_smooth(0, sweeps, dev(f), pg)
+    assert np.array_equal(po, host(pg))
+
+
+# --------------------------------------------------------------------------- #
 # V-cycles: every kernel-selection combination gives the oracle's iterate bit for bit
 # --------------------------------------------------------------------------- #
 OPTS = [dict(kernels=k, graph=gr, coarse_cta=c) for k, gr, c in itertools.product((0, 1), (0, 1), (0, 1))]
+OPTS += [dict(kernels=2, graph=1, coarse_cta=1), dict(kernels=1, graph=1, coarse_cta=1, tails=0),
+         dict(kernels=1, graph=0, coarse_cta=1, fuse=2)]
 
 
 @pytest.mark.parametrize("n,bc", SHAPES[:5] + SHAPES[7:])
-@pytest.mark.parametrize("opts", OPTS, ids=lambda d: "k%d-g%d-c%d" % (d["kernels"], d["graph"], d["coarse_cta"]))
+@pytest.mark.parametrize("opts", OPTS, ids=lambda d: "k%d-g%d-c%d-t%d-f%d" % (d["kernels"], d["graph"], d["coarse_cta"], d.get("tails", 1), d.get("fuse", 1)))
 @pytest.mark.parametrize("nu", [(2, 2), (3, 3), (1, 0)])
 def test_vcycle_bit_exact(mgmod, uniform, n, bc, opts, nu):
     h = 1.0 / n[0]
