@@ -9,18 +9,22 @@
 namespace mg {
 
 // ---- A0: coefficients -----------------------------------------------------
-// a = 0.5/rho (C2); flags[0] |= 1 if some rho is not a finite positive number.
+// a = 0.5/rho (C2); flags[0] |= 1 if some rho is not a finite positive number; flags[1] |= 1 if
+// some a lies outside [2^-900, 2^900].
 __global__ void k_cell_coef(const double *__restrict__ rho, double *__restrict__ a, size_t n,
                             int *__restrict__ flags)
 {
-    bool bad = false;
+    bool bad = false, wide = false;
     for (size_t c = blockIdx.x * (size_t)blockDim.x + threadIdx.x; c < n;
          c += (size_t)gridDim.x * blockDim.x) {
         const double r = rho[c];
         bad |= !(r > 0.0) || isinf(r);
-        a[c] = __ddiv_rn(0.5, r);
+        const double av = __ddiv_rn(0.5, r);
+        wide |= !(av >= 0x1p-900 && av <= 0x1p900);      // outside the range of the branch-free reciprocal
+        a[c] = av;
     }
     if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(flags, 1);
+    if (__syncthreads_or(wide) && threadIdx.x == 0) atomicOr(flags + 1, 1);
 }
 
 // minus faces of a CELL level written out explicitly (mg_level_faces on level 0)
