@@ -26,7 +26,7 @@ def main():
     ap.add_argument("--reps", type=int, default=5)
     ap.add_argument("--kernels", type=int, default=1)
     ap.add_argument("--graph", type=int, default=1)
-    ap.add_argument("--fuse", type=int, default=1)
+    ap.add_argument("--fuse", type=int, default=2)
     args = ap.parse_args()
     body = args.workload[len("config"):]
     cfg, n = (body.split("@") + [None])[:2]

@@ -157,14 +157,16 @@ def test_fused_norm_tail(mgmod, uniform, n, bc, sweeps):
     assert nrm == pytest.approx(o.residual(f, po), rel=NORM_RTOL)
 
 
+@pytest.mark.parametrize("fuse", [1, 2])
 @pytest.mark.parametrize("sweeps", [2, 4, 5])
-def test_two_sweeps_fused_per_pass_bit_exact(mgmod, uniform, sweeps):
-    """MG_OPT_SWEEP_FUSE = 2: temporal blocking, two red-black sweeps per pass of k_rbt<2>."""
+def test_two_sweeps_fused_per_pass_bit_exact(mgmod, uniform, sweeps, fuse):
+    """MG_OPT_SWEEP_FUSE = 2 (default): temporal blocking, two red-black sweeps per pass of
+    k_rbt<2>; = 1: one sweep per pass."""
     from paper_2605_30082_b200 import binding as B
     n, bc = (136, 72, 96), (P, N, P)
     shp = (n[2], n[1], n[0])
     o, g = pair(mgmod, n, 1.0 / n[0], bc, rho=random_rho(uniform, 57, shp))
-    g.set_option(B.MG_OPT_SWEEP_FUSE, 2)
+    g.set_option(B.MG_OPT_SWEEP_FUSE, fuse)
     f, p0 = uniform(58, shp), uniform(59, shp)
     po = p0.copy()
     for _ in range(sweeps):
@@ -179,11 +181,11 @@ def test_two_sweeps_fused_per_pass_bit_exact(mgmod, uniform, sweeps):
 # --------------------------------------------------------------------------- #
 OPTS = [dict(kernels=k, graph=gr, coarse_cta=c) for k, gr, c in itertools.product((0, 1), (0, 1), (0, 1))]
 OPTS += [dict(kernels=2, graph=1, coarse_cta=1), dict(kernels=1, graph=1, coarse_cta=1, tails=0),
-         dict(kernels=1, graph=0, coarse_cta=1, fuse=2)]
+         dict(kernels=1, graph=0, coarse_cta=1, fuse=1)]
 
 
 @pytest.mark.parametrize("n,bc", SHAPES[:5] + SHAPES[7:])
-@pytest.mark.parametrize("opts", OPTS, ids=lambda d: "k%d-g%d-c%d-t%d-f%d" % (d["kernels"], d["graph"], d["coarse_cta"], d.get("tails", 1), d.get("fuse", 1)))
+@pytest.mark.parametrize("opts", OPTS, ids=lambda d: "k%d-g%d-c%d-t%d-f%d" % (d["kernels"], d["graph"], d["coarse_cta"], d.get("tails", 1), d.get("fuse", 2)))
 @pytest.mark.parametrize("nu", [(2, 2), (3, 3), (1, 0)])
 def test_vcycle_bit_exact(mgmod, uniform, n, bc, opts, nu):
     h = 1.0 / n[0]
