@@ -44,7 +44,8 @@ def pair(mgmod, n, h, bc, nu=(2, 2), rho=None, coarse_sweeps=32, **opts):
     g = mgmod.Multigrid(n, h, bc, nu[0], nu[1], coarse_sweeps)
     from paper_2605_30082_b200 import binding as B
     for key, name in ((B.MG_OPT_KERNELS, "kernels"), (B.MG_OPT_GRAPH, "graph"), (B.MG_OPT_COARSE_CTA, "coarse_cta"),
-                      (B.MG_OPT_TAIL_FUSION, "tails"), (B.MG_OPT_SWEEP_FUSE, "fuse")):
+                      (B.MG_OPT_TAIL_FUSION, "tails"), (B.MG_OPT_SWEEP_FUSE, "fuse"),
+                      (B.MG_OPT_FACE_STREAM_LOG2, "face_log2")):
         if name in opts:
             g.set_option(key, opts[name])
     if rho is not None:
@@ -174,6 +175,61 @@ def test_two_sweeps_fused_per_pass_bit_exact(mgmod, uniform, sweeps, fuse):
     pg = dev(p0)
     g.level_smooth(0, sweeps, dev(f), pg)
     assert np.array_equal(po, host(pg))
+
+
+# --------------------------------------------------------------------------- #
+# the TMA sweep kernel on the stored-face levels (>= 1): forced onto small levels with
+# MG_OPT_FACE_STREAM_LOG2 = 0 (by default only levels of 2^20 cells and more take it).
+# Sweeps, fused pairs of sweeps and the restriction tail bit-exact on level 1 and 2;
+# periodic wrap (patched images), walls (zero fill, masked updates) and ragged tiles.
+# --------------------------------------------------------------------------- #
+FACE_SHAPES = [
+    ((64, 64, 64), (P, P, P)),
+    ((64, 64, 64), (N, N, N)),
+    ((136, 72, 96), (N, P, P)),
+    ((80, 144, 64), (P, N, N)),
+    ((128, 128, 128), (P, P, N)),     # level 1 = 64^3 and level 2 = 32^3 both stream
+]
+
+
+@pytest.mark.parametrize("n,bc", FACE_SHAPES)
+@pytest.mark.parametrize("fuse", [1, 2])
+def test_face_levels_streamed_bit_exact(mgmod, uniform, n, bc, fuse):
+    shp = (n[2], n[1], n[0])
+    o, g = pair(mgmod, n, 1.0 / n[0], bc, rho=random_rho(uniform, 61, shp), fuse=fuse, face_log2=0)
+    for lvl in range(1, o.num_levels - 1):
+        lshp = o.level_shape(lvl)                      # (nz, ny, nx)
+        if min(lshp[1], lshp[2]) < 32 or lshp[0] < 16:
+            break
+        f, p0 = uniform(62 + lvl, lshp), uniform(66 + lvl, lshp)
+        fd = dev(f)
+        for sweeps in (1, 2, 3, 4):
+            po = p0.copy()
+            for _ in range(sweeps):
+                o.sweep(f, po, lvl)
+            pg = dev(p0)
+            g.level_smooth(lvl, sweeps, fd, pg)
+            assert np.array_equal(po, host(pg)), f"level {lvl}, {sweeps} sweeps"
+            # the same sweeps with residual + restriction fused behind the last one
+            fc_o = o.restrict(o.residual_level(f, po, lvl), lvl)
+            pg = dev(p0)
+            fc_g = g.level_smooth_restrict(lvl, sweeps, fd, pg)
+            assert np.array_equal(po, host(pg)), f"level {lvl}, {sweeps} sweeps + tail: p"
+            assert np.array_equal(fc_o, host(fc_g)), f"level {lvl}, {sweeps} sweeps + tail: coarse rhs"
+
+
+@pytest.mark.parametrize("n,bc", FACE_SHAPES)
+@pytest.mark.parametrize("nu", [(2, 2), (3, 3)])
+def test_vcycle_face_levels_streamed_bit_exact(mgmod, uniform, n, bc, nu):
+    shp = (n[2], n[1], n[0])
+    o, g = pair(mgmod, n, 1.0 / n[0], bc, nu=nu, rho=random_rho(uniform, 71, shp), coarse_sweeps=8, face_log2=0)
+    f = uniform(72, shp)
+    f -= f.mean()
+    po, pg, fd = np.zeros(shp), dev(np.zeros(shp)), dev(f)
+    for cyc in range(2):
+        o.vcycle(f, po)
+        g.vcycle(fd, pg)
+        assert np.array_equal(po, host(pg)), f"cycle {cyc}"
 
 
 # --------------------------------------------------------------------------- #
