@@ -70,7 +70,7 @@ enum {
                                0 = separate passes */
     MG_OPT_FACE_STREAM_LOG2 = 6 /* stored-face levels (>= 1) with at least 2^value cells use the
                                TMA kernel, smaller ones two half-sweep launches per sweep
-                               (default 20; 0 = every level the kernel can tile) */
+                               (default 24; 0 = every level the kernel can tile) */
 };
 
 /* mg_get_stat keys */
