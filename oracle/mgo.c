@@ -31,6 +31,7 @@ struct mgo_solver {
     int nlev;
     int bc[3];
     int nu1, nu2, coarse_sweeps;
+    int cycle_type;             /* R23: MGO_CYCLE_V / F / W */
     level_t lv[MGO_MAX_LEVELS];
 };
 
@@ -316,7 +317,12 @@ static long double sum_planes(const level_t *L, const double *x, int squared)
 }
 
 /* ------------------------------------------------------------------ cycle */
-static void vcycle(mgo_solver *s, int l, double *p, const double *f)
+/* One multigrid cycle on level l (SURVEY 8(c) "Oracle algorithm"; cycle index per Brandt /
+ * Trottenberg et al., DESIGN R23).  type V: the coarse problem is visited once.  type W: twice,
+ * the second visit starting from the correction the first one left.  type F: an F-cycle visit
+ * followed by a V-cycle visit.  The coarsest level is a fixed number of sweeps (R13) and is
+ * visited once per visit of the level above it. */
+static void cycle(mgo_solver *s, int l, double *p, const double *f, int type)
 {
     level_t *L = &s->lv[l];
     if (l == s->nlev - 1) {                                  /* R13 */
@@ -328,9 +334,25 @@ static void vcycle(mgo_solver *s, int l, double *p, const double *f)
     residual(L, f, p, L->r);
     restrict8(L, C, L->r, C->f);
     memset(C->p, 0, lv_cells(C) * sizeof(double));
-    vcycle(s, l + 1, C->p, C->f);
+    cycle(s, l + 1, C->p, C->f, type);
+    if (l + 1 < s->nlev - 1) {
+        if (type == MGO_CYCLE_W) cycle(s, l + 1, C->p, C->f, MGO_CYCLE_W);
+        if (type == MGO_CYCLE_F) cycle(s, l + 1, C->p, C->f, MGO_CYCLE_V);
+    }
     prolong_add(s, L, C, C->p, p);
     for (int it = 0; it < s->nu2; ++it) sweep(L, f, p);
+}
+
+static void vcycle(mgo_solver *s, int l, double *p, const double *f)
+{
+    cycle(s, l, p, f, s->cycle_type);
+}
+
+int mgo_set_cycle_type(mgo_solver *s, int type)
+{
+    if (!s || type < MGO_CYCLE_V || type > MGO_CYCLE_W) return MGO_EINVAL;
+    s->cycle_type = type;
+    return MGO_OK;
 }
 
 int mgo_vcycle(mgo_solver *s, const double *rhs, double *p)

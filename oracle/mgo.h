@@ -53,6 +53,11 @@ enum { MGO_OK = 0, MGO_NOT_CONVERGED = 1, MGO_EINVAL = -1, MGO_ENOMEM = -2,
 int  mgo_create(int nx, int ny, int nz, double h, const int bc[3], mgo_solver **out);
 void mgo_destroy(mgo_solver *s);
 int  mgo_set_cycle(mgo_solver *s, int nu1, int nu2, int coarse_sweeps);
+/* R23: cycle index.  V (default): one visit of the coarse problem per level;
+ * W: two, the second continuing from the first one's correction; F: an F visit, then a V visit.
+ * mgo_vcycle / mgo_solve run this cycle. */
+enum { MGO_CYCLE_V = 0, MGO_CYCLE_F = 1, MGO_CYCLE_W = 2 };
+int  mgo_set_cycle_type(mgo_solver *s, int type);
 int  mgo_set_density(mgo_solver *s, const double *rho);
 
 int  mgo_vcycle(mgo_solver *s, const double *rhs, double *p);

@@ -65,6 +65,7 @@ def lib():
         L.mgo_destroy.argtypes = [vp]
         L.mgo_destroy.restype = None
         L.mgo_set_cycle.argtypes = [vp, C.c_int, C.c_int, C.c_int]
+        L.mgo_set_cycle_type.argtypes = [vp, C.c_int]
         L.mgo_set_density.argtypes = [vp, dp]
         L.mgo_vcycle.argtypes = [vp, dp, dp]
         L.mgo_residual.argtypes = [vp, dp, dp, dp, dp]
@@ -153,6 +154,10 @@ class Oracle:
     # ---- the calls of the boundary
     def set_cycle(self, nu1, nu2, coarse_sweeps=32):
         _chk(lib().mgo_set_cycle(self._h, nu1, nu2, coarse_sweeps))
+
+    def set_cycle_type(self, type):
+        """0 = V (default), 1 = F, 2 = W (R23)."""
+        _chk(lib().mgo_set_cycle_type(self._h, int(type)))
 
     def set_density(self, rho):
         _chk(lib().mgo_set_density(self._h, _dp(self._arr(rho))))
