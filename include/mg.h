@@ -106,6 +106,15 @@ int mg_set_stream(mg_handle *s, void *cuda_stream);
 /* V(nu1,nu2) and the number of sweeps on the coarsest level (defaults 2,2,32). */
 int mg_set_cycle(mg_handle *s, int nu1, int nu2, int coarse_sweeps);
 
+/* Cycle index (R23; the paper only names "the Multigrid",
+ * PAPER.md:216).  MG_CYCLE_V (default): every level visits its coarse problem once.
+ * MG_CYCLE_W: twice, the second visit continuing from the correction of the first.
+ * MG_CYCLE_F: an F-cycle visit followed by a V-cycle visit.  The coarsest level (R13) is
+ * visited once per visit of the level above it.  mg_vcycle, mg_solve and mg_project run this
+ * cycle; changing it re-captures the graph.  MG_EINVAL for any other value. */
+enum { MG_CYCLE_V = 0, MG_CYCLE_F = 1, MG_CYCLE_W = 2 };
+int mg_set_cycle_type(mg_handle *s, int type);
+
 int mg_set_option(mg_handle *s, int key, int value);
 int mg_get_stat(const mg_handle *s, int key, long long *value_host);
 

@@ -26,6 +26,7 @@ SIGNATURES = {
     "mg_create_in": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_double, _ip, _vp, C.c_size_t, C.POINTER(_vp)]),
     "mg_destroy": (None, [_vp]),
     "mg_set_stream": (C.c_int, [_vp, _vp]),
+    "mg_set_cycle_type": (C.c_int, [_vp, C.c_int]),
     "mg_set_cycle": (C.c_int, [_vp, C.c_int, C.c_int, C.c_int]),
     "mg_set_option": (C.c_int, [_vp, C.c_int, C.c_int]),
     "mg_get_stat": (C.c_int, [_vp, C.c_int, C.POINTER(C.c_longlong)]),
@@ -146,6 +147,10 @@ class Multigrid:
     # ---- configuration
     def set_cycle(self, nu1, nu2, coarse_sweeps=32):
         _chk(lib().mg_set_cycle(self._h, nu1, nu2, coarse_sweeps))
+
+    def set_cycle_type(self, type):
+        """0 = V (default), 1 = F, 2 = W."""
+        _chk(lib().mg_set_cycle_type(self._h, int(type)))
 
     def set_option(self, key, value):
         _chk(lib().mg_set_option(self._h, key, value))

@@ -31,8 +31,10 @@ struct CoarseArgs {
     const double *bx[kCoarseMaxLevels], *by[kCoarseMaxLevels], *bz[kCoarseMaxLevels];
     int bc[3];
     int nu1, nu2, coarse_sweeps;
+    int cycle_type;      // 0 = V, 1 = F, 2 = W (R23)
+    int warm;            // 0: initial guess 0; 1: a later visit, the guess is read from p
     const double *f;     // rhs of the top level handled here (global, read once)
-    double *p;           // correction of that level (global, written once; initial guess is 0)
+    double *p;           // correction of that level (global, written once)
 };
 
 inline size_t coarse_cta_bytes(int (*n)[3], int nlev)
@@ -169,6 +171,46 @@ __device__ __forceinline__ void coarse_prolong_add(const CLv &L, const CLv &C, c
     }
 }
 
+// F- and W-cycles (R23) below the top level of the CTA: the recursion of the cycle index walked
+// with an explicit stack (at most kCoarseMaxLevels frames), every thread of the CTA in step.
+// A frame is (level, cycle type, stage): 0 = entered, 1 = first visit of the coarse problem done,
+// 2 = both done.
+__device__ __forceinline__ void coarse_cycle(const CoarseArgs &A, double *sm, int type, int tid, int nthr)
+{
+    int fq[kCoarseMaxLevels + 1], fty[kCoarseMaxLevels + 1], fst[kCoarseMaxLevels + 1];
+    int sp = 0;
+    fq[0] = 0; fty[0] = type; fst[0] = 0;
+    while (sp >= 0) {
+        const int q = fq[sp], ty = fty[sp];
+        const CLv L = coarse_level(A, q, sm);
+        if (q == A.nlev - 1) {                               // R13
+            coarse_sweeps(L, A.coarse_sweeps, tid, nthr);
+            --sp;
+            continue;
+        }
+        const CLv C = coarse_level(A, q + 1, sm);
+        if (fst[sp] == 0) {
+            coarse_sweeps(L, A.nu1, tid, nthr);
+            coarse_residual_restrict(L, C, tid, nthr);
+            __syncthreads();
+            fst[sp] = 1;
+            ++sp; fq[sp] = q + 1; fty[sp] = ty; fst[sp] = 0;
+            continue;
+        }
+        if (fst[sp] == 1) {
+            fst[sp] = 2;
+            if (q + 1 < A.nlev - 1 && ty != 0) {             // second visit: W again, or V after F
+                ++sp; fq[sp] = q + 1; fty[sp] = ty == 2 ? 2 : 0; fst[sp] = 0;
+                continue;
+            }
+        }
+        coarse_prolong_add(L, C, A.bc, tid, nthr);
+        __syncthreads();
+        coarse_sweeps(L, A.nu2, tid, nthr);
+        --sp;
+    }
+}
+
 __global__ void __launch_bounds__(kCoarseThreads, 1) k_coarse_cta(CoarseArgs A)
 {
     extern __shared__ __align__(16) double coarse_sm[];
@@ -181,7 +223,7 @@ __global__ void __launch_bounds__(kCoarseThreads, 1) k_coarse_cta(CoarseArgs A)
         const double *gx = A.bx[q], *gy = A.by[q], *gz = A.bz[q];
         for (int c = tid; c < n; c += nthr) {
             L.bx[c] = gx[c]; L.by[c] = gy[c]; L.bz[c] = gz[c];
-            if (q == 0) { L.f[c] = A.f[c]; L.p[c] = 0.0; }
+            if (q == 0) { L.f[c] = A.f[c]; L.p[c] = A.warm ? A.p[c] : 0.0; }
         }
     }
     __syncthreads();
@@ -195,6 +237,9 @@ __global__ void __launch_bounds__(kCoarseThreads, 1) k_coarse_cta(CoarseArgs A)
     }
     __syncthreads();
 
+    if (A.cycle_type != 0) {
+        coarse_cycle(A, coarse_sm, A.cycle_type, tid, nthr);
+    } else {
     // ---- down
     for (int q = 0; q + 1 < A.nlev; ++q) {
         const CLv L = coarse_level(A, q, coarse_sm);
@@ -215,6 +260,7 @@ __global__ void __launch_bounds__(kCoarseThreads, 1) k_coarse_cta(CoarseArgs A)
         coarse_prolong_add(L, C, A.bc, tid, nthr);
         __syncthreads();
         coarse_sweeps(L, A.nu2, tid, nthr);
+    }
     }
     // ---- correction of the top level back to global memory
     {

@@ -48,6 +48,9 @@ def pair(mgmod, n, h, bc, nu=(2, 2), rho=None, coarse_sweeps=32, **opts):
                       (B.MG_OPT_FACE_STREAM_LOG2, "face_log2")):
         if name in opts:
             g.set_option(key, opts[name])
+    if "cycle_type" in opts:
+        o.set_cycle_type(opts["cycle_type"])
+        g.set_cycle_type(opts["cycle_type"])
     if rho is not None:
         o.set_density(rho)
         g.set_density(dev(rho))
@@ -256,6 +259,38 @@ def test_vcycle_bit_exact(mgmod, uniform, n, bc, opts, nu):
         g.vcycle(fd, pg)
         assert np.array_equal(po, host(pg)), f"cycle {cyc}"
     assert g.residual(fd, pg) == pytest.approx(o.residual(f, po), rel=NORM_RTOL)
+
+
+# --------------------------------------------------------------------------- #
+# F- and W-cycles (mg_set_cycle_type, DESIGN R23): the iterate of every
+# cycle bit for bit, with the levels <= 16^3 inside the coarse CTA (its own recursion) and
+# launch by launch, graph and no graph; then whole solves
+# --------------------------------------------------------------------------- #
+CYCLE_SHAPES = [((32, 32, 32), (P, P, N)), ((64, 64, 64), (N, P, N)), ((72, 40, 36), (P, N, N)),
+                ((128, 128, 128), (P, P, P))]
+
+
+@pytest.mark.parametrize("n,bc", CYCLE_SHAPES)
+@pytest.mark.parametrize("cycle_type", [1, 2], ids=["F", "W"])
+@pytest.mark.parametrize("opts", [dict(), dict(coarse_cta=0, graph=0), dict(kernels=0), dict(face_log2=0)],
+                         ids=["default", "no-cta-no-graph", "reference-kernels", "faces-streamed"])
+def test_f_and_w_cycles_bit_exact(mgmod, uniform, n, bc, cycle_type, opts):
+    shp = (n[2], n[1], n[0])
+    o, g = pair(mgmod, n, 1.0 / n[0], bc, nu=(2, 1), rho=random_rho(uniform, 91, shp), coarse_sweeps=6,
+                cycle_type=cycle_type, **opts)
+    f = uniform(92, shp)
+    f -= f.mean()
+    po, pg, fd = np.zeros(shp), dev(np.zeros(shp)), dev(f)
+    for cyc in range(3):
+        o.vcycle(f, po)
+        g.vcycle(fd, pg)
+        assert np.array_equal(po, host(pg)), f"cycle {cyc}"
+
+
+@pytest.mark.parametrize("cycle_type", [1, 2], ids=["F", "W"])
+@pytest.mark.parametrize("cfg,n", [(3, 64), (3, 128), (2, 64)])
+def test_solve_with_f_and_w_cycles(mgmod, cfg, n, cycle_type):
+    check_solve(mgmod, make_workload(cfg, n), cycle_type=cycle_type)
 
 
 # --------------------------------------------------------------------------- #
