@@ -41,7 +41,6 @@ UNIT = "Gcell-updates/s"
 # algorithmic HBM bytes: level-0 sweep pass 32 B/cell
 # (p read+write, f, a); coarse-level pass 48 B/cell; whole V(3,3) cycle per fine cell:
 B_SWEEP_L0 = 32.0
-NCU_SWEEP_TRAFFIC_512 = 3.633e9 + 1.050e9     # bytes per launch (algorithmic: 4.295e9)
 
 
 def b_sched_per_fine_cell(nu1, nu2):
@@ -67,6 +66,12 @@ def parse_workload(name: str):
         c, n = body.split("@")
         return int(c), int(n)
     return int(body), None
+
+
+def workload_config(w, wname):
+    """The keys of `config` that identify the workload: the same in both arms."""
+    return {"workload": wname, "cells": list(w.n), "bc": list(w.bc), "cycle": f"V({w.nu1},{w.nu2})",
+            "rtol": w.rtol, "step": "mg_set_density + mg_solve from p=0", "parallelism": "replicas only"}
 
 
 def peaks():
@@ -155,12 +160,13 @@ def run_reference(args, w, wname):
     t = times[args.warmup:]
     per = float(np.mean(t))
     val = w.ncells * (w.nu1 + w.nu2) / per / 1e9
-    sample = f"1 V({w.nu1},{w.nu2}) cycle + 1 residual norm per step on {wname} (of ~12 cycles per solve)"
+    sample = (f"1 V({w.nu1},{w.nu2}) cycle + 1 residual norm per step on {wname} "
+              "(a bounded sample of the step: the solve is 17 such cycles at 512^3)")
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": per * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": wname, "cells": list(w.n), "cycle": f"V({w.nu1},{w.nu2})", "rtol": w.rtol},
+        "config": workload_config(w, wname),
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": thr, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -201,23 +207,34 @@ def aggregate_replicas(times_ms, counts, dist, device):
     return t.tolist(), c.tolist()
 
 
-def run_cuda(args, w, wname):
+def free_port():
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        return sk.getsockname()[1]
+
+
+def spawn_command(args, argv, environ):
+    """`--gpus N` without a launcher: the command that runs this script as N ranks (one per GPU),
+    or None when a launcher already did (WORLD_SIZE set) or one GPU is asked for."""
+    if args.gpus <= 1 or "WORLD_SIZE" in environ:
+        return None
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+            "--master-addr", "127.0.0.1", "--master-port", str(free_port()), str(ROOT / "bench.py"), *argv]
+
+
+def measure_rank(args, w, wname, rank, local, dist):
+    """Everything one rank measures on its own GPU (CUDA events on the solver's stream)."""
     import torch
 
     import paper_2605_30082_b200 as mgpkg
     from paper_2605_30082_b200 import binding as B
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     torch.cuda.set_device(local)
     devname = f"cuda:{local}"
     N = w.ncells
     stream = torch.cuda.Stream(device=devname)
+    m = {}
 
     with torch.cuda.stream(stream):
         g = mgpkg.Multigrid(w.n, w.h, w.bc, w.nu1, w.nu2, stream=stream, device=devname)
@@ -225,6 +242,7 @@ def run_cuda(args, w, wname):
         rhs_d = torch.from_numpy(w.rhs).to(devname)
         p_d = torch.zeros(g.shape, dtype=torch.float64, device=devname)
         max_cycles = 60
+        m["levels"] = g.num_levels
 
         def barrier():
             torch.cuda.synchronize()
@@ -250,47 +268,63 @@ def run_cuda(args, w, wname):
                 cycles_total += res[1]
             ev1.record(stream)
             barrier()
-        t_ms = ev0.elapsed_time(ev1)
-        launches = g.stat(B.MG_STAT_KERNEL_LAUNCHES) - l0
-        status, cycles, relres, hist = res
+        m["t_ms"] = ev0.elapsed_time(ev1)
+        m["cycles_total"] = cycles_total
+        m["launches"] = g.stat(B.MG_STAT_KERNEL_LAUNCHES) - l0
+        m["status"], m["cycles"], m["relres"], _ = res
+        m["clocks"] = clocks.summary()
 
-        # time-to-rtol: mg_solve alone
+        def timed(fn, reps, warm=2):
+            for _ in range(warm):
+                fn()
+            torch.cuda.synchronize()
+            lk = g.stat(B.MG_STAT_KERNEL_LAUNCHES)
+            ev0.record(stream)
+            for _ in range(reps):
+                fn()
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            return ev0.elapsed_time(ev1) / reps, (g.stat(B.MG_STAT_KERNEL_LAUNCHES) - lk) / reps
+
+        # time-to-rtol: mg_solve alone, with the V-cycle of the config and with the F-cycle
+        def solve_once():
+            p_d.zero_()
+            return g.solve(rhs_d, p_d, w.rtol, max_cycles)
+
         g.set_density(rho_d)
+        m["t_solve_ms"], _ = timed(solve_once, 1, warm=0)
+        g.set_cycle_type(B.MG_CYCLE_F)
+        solve_once()
+        t_f, _ = timed(solve_once, 1, warm=0)
+        rf = solve_once()
         p_d.zero_()
-        torch.cuda.synchronize()
-        ev0.record(stream)
-        g.solve(rhs_d, p_d, w.rtol, max_cycles)
-        ev1.record(stream)
-        torch.cuda.synchronize()
-        t_solve_ms = ev0.elapsed_time(ev1)
+        t_fc, _ = timed(lambda: g.vcycle(rhs_d, p_d), 10, warm=3)
+        m["f_cycle"] = {"time_to_rtol_ms": t_f, "cycles": rf[1], "relres": rf[2], "ms_per_cycle": t_fc,
+                        "what": "the same solve with mg_set_cycle_type(MG_CYCLE_F): F(nu1,nu2) cycles"}
+        g.set_cycle_type(B.MG_CYCLE_V)
 
         # bare V-cycle (graph replay), 20 launches after 3 warm-ups
         p_d.zero_()
-        for _ in range(3):
-            g.vcycle(rhs_d, p_d)
-        torch.cuda.synchronize()
-        ev0.record(stream)
-        for _ in range(20):
-            g.vcycle(rhs_d, p_d)
-        ev1.record(stream)
-        torch.cuda.synchronize()
-        t_vc_ms = ev0.elapsed_time(ev1) / 20
-        launches_per_vcycle = g.stat(B.MG_STAT_LAUNCHES_PER_VCYCLE)
+        m["t_vc_ms"], _ = timed(lambda: g.vcycle(rhs_d, p_d), 20, warm=3)
+        m["launches_per_vcycle"] = g.stat(B.MG_STAT_LAUNCHES_PER_VCYCLE)
 
-        # dominant kernel: level-0 red-black sweep pass, CUDA events on the launching stream
+        # the kernels of level 0, one by one (CUDA events on the launching stream; every call
+        # below is one or two launches of the named kernel, counted by the library)
+        kern = {}
         p_d.zero_()
-        # (two sweeps per call = two launches of the streaming kernel, p -> q -> p)
-        for _ in range(3):
-            g.level_smooth(0, 2, rhs_d, p_d)
-        torch.cuda.synchronize()
-        lk0 = g.stat(B.MG_STAT_KERNEL_LAUNCHES)
-        ev0.record(stream)
-        for _ in range(10):
-            g.level_smooth(0, 2, rhs_d, p_d)
-        ev1.record(stream)
-        torch.cuda.synchronize()
-        t_sweep_ms = ev0.elapsed_time(ev1) / 20
-        launches_per_sweep = (g.stat(B.MG_STAT_KERNEL_LAUNCHES) - lk0) / 20
+        t, nl = timed(lambda: g.level_smooth(0, 4, rhs_d, p_d), 10)
+        kern["k_rbt<NS=2> two sweeps per pass"] = {"ms": t / nl, "bytes_per_cell": 32.0, "sweeps_per_launch": 2}
+        g.set_option(B.MG_OPT_SWEEP_FUSE, 1)
+        t, nl = timed(lambda: g.level_smooth(0, 2, rhs_d, p_d), 10)
+        kern["k_rbt<NS=1> one sweep per pass"] = {"ms": t / nl, "bytes_per_cell": 32.0, "sweeps_per_launch": 1}
+        g.set_option(B.MG_OPT_SWEEP_FUSE, 2)
+        e1_d = torch.zeros(g.level_shape(1), dtype=torch.float64, device=devname)
+        t, nl = timed(lambda: g.level_prolong_add(0, e1_d, p_d), 10)
+        kern["k_prolong_stream"] = {"ms": t / nl, "bytes_per_cell": 17.0}
+        t, nl = timed(lambda: g.residual(rhs_d, p_d), 10)
+        kern["k_resid_stream<NORM> (+ k_final_sum)"] = {"ms": t, "bytes_per_cell": 24.0}
+        del e1_d
+        m["kernels"] = kern
 
         # set_density alone
         torch.cuda.synchronize()
@@ -298,7 +332,7 @@ def run_cuda(args, w, wname):
         g.set_density(rho_d)
         ev1.record(stream)
         torch.cuda.synchronize()
-        t_setrho_ms = ev0.elapsed_time(ev1)
+        m["t_setrho_ms"] = ev0.elapsed_time(ev1)
 
         # the projection step around the solve: rhs = div(u*)/dt,
         # solve, u -= dt beta grad p, on the 16-mode staggered velocity behind the workload's rhs
@@ -386,56 +420,101 @@ def run_cuda(args, w, wname):
             e2e_cycles += g.solve_host(rho_h, rhs_h, p_h, w.rtol, max_cycles)[1]
         ev1.record(stream)
         barrier()
-        t_e2e_ms = ev0.elapsed_time(ev1)
+        m["t_e2e_ms"] = ev0.elapsed_time(ev1)
+        m["e2e_cycles"], m["e2e_steps"] = e2e_cycles, e2e_steps
+    m["proj"], m["seq"] = proj, seq
+    return m
 
-    # max over ranks of the times, sum over ranks of the units
-    (t_ms, t_e2e_ms), (cycles_all, e2e_cycles_all) = aggregate_replicas(
-        [t_ms, t_e2e_ms], [float(cycles_total), float(e2e_cycles)], dist, devname)
-    if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
-        return
 
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel at 512^3, from the
+# `ncu --set full` capture summarised in the named file (bench.py itself never runs under ncu)
+NCU_TRAFFIC_512 = {"bytes": 4.272e9 + 1.114e9, "source": "profiles/r2b_cycle.md (k_rbt<NS=2>, 512^3)"}
+
+
+def assemble_line(args, w, wname, world, m, t_ms, t_e2e_ms, cycles_all, e2e_cycles_all):
+    """The JSON line from rank 0's measurements and the aggregated (max time, summed units)."""
+    N = w.ncells
     upd = w.nu1 + w.nu2
     value = N * upd * cycles_all / (t_ms * 1e-3) / 1e9
     e2e_value = N * upd * e2e_cycles_all / (t_e2e_ms * 1e-3) / 1e9
     peak, peak_src = peaks()
-    sweep_bytes = B_SWEEP_L0 * N
-    achieved = sweep_bytes / (t_sweep_ms * 1e-3) / 1e9
     bs = b_sched_per_fine_cell(w.nu1, w.nu2) * N
     bw = b_sweep_per_fine_cell(w.nu1, w.nu2) * N
+    t_vc_ms = m["t_vc_ms"]
+    # per-kernel HBM roofline: algorithmic bytes of one launch / event-timed launch duration
+    kernels = {}
+    for name, k in m.get("kernels", {}).items():
+        ach = k["bytes_per_cell"] * N / (k["ms"] * 1e-3) / 1e9
+        kernels[name] = dict(k, achieved_gbs=ach, frac=ach / peak)
+    dom_name = "k_rbt<NS=2> two sweeps per pass"
+    dom = kernels.get(dom_name)
+    roof = {"bound": "hbm", "kernel": dom_name + " (level 0, p_in -> p_out: 32 B/cell per launch)",
+            "achieved": dom["achieved_gbs"] if dom else None, "peak": peak, "unit": "GB/s",
+            "frac": dom["frac"] if dom else None, "traffic": None, "peak_source": peak_src,
+            "bytes_per_launch": 32.0 * N, "ms_per_launch": dom["ms"] if dom else None,
+            "note": "dominant by share of the V-cycle (2 launches); two red-black sweeps per HBM pass, so "
+                    "its bytes per second are lower than the one-sweep pass's although each sweep is faster: "
+                    "the fused pass is bound by shared-memory bandwidth and latency, not by HBM (DESIGN.md 4.1)",
+            "per_sweep_equivalent_frac": (2 * dom["frac"]) if dom else None,
+            "kernels": kernels}
+    if list(w.n) == [512, 512, 512]:
+        roof["traffic"] = NCU_TRAFFIC_512["bytes"]
+        roof["traffic_source"] = NCU_TRAFFIC_512["source"]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": t_ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": wname, "cells": list(w.n), "bc": list(w.bc), "cycle": f"V({w.nu1},{w.nu2})",
-                   "rtol": w.rtol, "levels": g.num_levels, "cycles_per_solve": cycles, "relres": relres,
-                   "step": "mg_set_density + mg_solve from p=0", "l2": "inputs larger than L2 "
-                   f"({3 * N * 8 / 1e6:.0f} MB resident vs 126 MB)", "parallelism": "replicas only"},
-        "time_to_rtol_ms": t_solve_ms, "set_density_ms": t_setrho_ms,
+        "config": workload_config(w, wname),
+        "solve": {"levels": m["levels"], "cycles_per_solve": m["cycles"], "relres": m["relres"],
+                  "l2": f"inputs larger than L2 ({3 * N * 8 / 1e6:.0f} MB resident vs 126 MB)"},
+        "time_to_rtol_ms": m["t_solve_ms"], "set_density_ms": m["t_setrho_ms"],
+        "f_cycle": m.get("f_cycle"),
         "vcycle": {"ms": t_vc_ms, "gcell_updates_per_s": N * upd / (t_vc_ms * 1e-3) / 1e9,
-                   "launches": launches_per_vcycle,
+                   "launches": m["launches_per_vcycle"],
                    "frac_of_B_sched_roofline": (bs / (peak * 1e9)) / (t_vc_ms * 1e-3),
                    "frac_of_B_sweep_roofline": (bw / (peak * 1e9)) / (t_vc_ms * 1e-3),
                    "B_sched_bytes": bs, "B_sweep_bytes": bw},
-        "roofline": {"bound": "hbm", "kernel": "k_sweep3<CELL> (level-0 red-black sweep pass, p_in -> p_out)", "achieved": achieved,
-                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
-                     "peak_source": peak_src, "bytes_per_launch": sweep_bytes,
-                     "ms_per_sweep": t_sweep_ms, "launches_per_sweep": launches_per_sweep},
+        "roofline": roof,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * N * 8, "d2h_bytes_per_step": N * 8,
-                "ms_per_step": t_e2e_ms / e2e_steps, "steps": e2e_steps, "api": "mg_solve_host (pinned host buffers)"},
-        "gpu_launches": int(launches),
-        "clocks": clocks.summary(),
+                "ms_per_step": t_e2e_ms / m["e2e_steps"], "steps": m["e2e_steps"],
+                "api": "mg_solve_host (pinned host buffers)"},
+        "gpu_launches": int(m["launches"]),
+        "clocks": m["clocks"],
     }
-    if proj is not None:
-        line["projection_step"] = proj
-    if seq is not None:
-        line["time_sequence"] = seq
-    # dram__bytes_read.sum + dram__bytes_write.sum of one k_sweep3<CELL> launch from the
-    # `ncu --set full` capture summarised in profiles/r1d_cycle.md (512^3 only)
-    if list(w.n) == [512, 512, 512]:
-        line["roofline"]["traffic"] = NCU_SWEEP_TRAFFIC_512
+    if m.get("proj") is not None:
+        line["projection_step"] = m["proj"]
+    if m.get("seq") is not None:
+        line["time_sequence"] = m["seq"]
+    return line
+
+
+def run_cuda(args, w, wname, measure=measure_rank, backend="nccl"):
+    """One process per GPU: every rank measures its own replica (`measure`), the job's time is the
+    MAX over ranks and its work the SUM (aggregate_replicas), rank 0 prints the line."""
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    device = "cpu"
+    if world > 1:
+        import torch.distributed as dist
+        if backend == "nccl":
+            import torch
+            dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+        else:
+            dist.init_process_group(backend)
+    if backend == "nccl":
+        device = f"cuda:{local}"
+    m = measure(args, w, wname, rank, local, dist)
+    (t_ms, t_e2e_ms), (cycles_all, e2e_cycles_all) = aggregate_replicas(
+        [m["t_ms"], m["t_e2e_ms"]], [float(m["cycles_total"]), float(m["e2e_cycles"])], dist, device)
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    line = assemble_line(args, w, wname, world, m, t_ms, t_e2e_ms, cycles_all, e2e_cycles_all)
     if world == 1 and not args.no_cpu_baseline:
+        N, upd, cycles = w.ncells, w.nu1 + w.nu2, m["cycles"]
         times_o, thr = oracle_sample(w, repeats=1, min_seconds=10.0)
         line["cpu_baseline"] = {
             "value": N * upd * len(times_o) / sum(times_o) / 1e9, "unit": UNIT, "cores": thr, "kind": "oracle",
@@ -463,6 +542,9 @@ def main():
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3
+    cmd = spawn_command(args, sys.argv[1:], os.environ) if args.impl == "cuda" else None
+    if cmd is not None:                 # --gpus N without a launcher: run N ranks, one per GPU
+        raise SystemExit(subprocess.run(cmd).returncode)
     from workloads import make_workload
 
     cfg, n = parse_workload(args.workload)

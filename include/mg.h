@@ -60,8 +60,7 @@ enum { MG_BC_PERIODIC = 0, MG_BC_NEUMANN = 1 };
 /* mg_set_option keys */
 enum {
     MG_OPT_KERNELS = 1,     /* 0 = reference kernels (one launch per half-sweep / transfer),
-                               1 = fused streaming kernels, TMA-staged sweeps on level 0 (default),
-                               2 = as 1 with the cp.async register-ring sweep of round 1     */
+                               1 = fused streaming kernels, TMA-staged sweeps (default)      */
     MG_OPT_GRAPH = 2,       /* 1 (default) = V-cycle replayed from a captured CUDA graph     */
     MG_OPT_COARSE_CTA = 3,  /* 1 (default) = levels <= 16^3 run in one persistent CTA       */
     MG_OPT_SWEEP_FUSE = 4,  /* sweeps fused per pass of the TMA kernel: 1 or 2 (default) */

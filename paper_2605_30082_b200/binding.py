@@ -15,6 +15,7 @@ MG_EINVAL, MG_ENOMEM, MG_ECUDA, MG_EINCOMPATIBLE, MG_EDIVERGED = -1, -2, -3, -4,
 MG_BC_PERIODIC, MG_BC_NEUMANN = 0, 1
 MG_OPT_KERNELS, MG_OPT_GRAPH, MG_OPT_COARSE_CTA, MG_OPT_SWEEP_FUSE, MG_OPT_TAIL_FUSION = 1, 2, 3, 4, 5
 MG_OPT_FACE_STREAM_LOG2 = 6
+MG_CYCLE_V, MG_CYCLE_F, MG_CYCLE_W = 0, 1, 2
 MG_STAT_KERNEL_LAUNCHES, MG_STAT_WORKSPACE_BYTES, MG_STAT_LAUNCHES_PER_VCYCLE = 1, 2, 3
 
 _vp, _dp, _ip = C.c_void_p, C.c_void_p, C.POINTER(C.c_int)   # device pointers travel as integers

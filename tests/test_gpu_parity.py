@@ -239,7 +239,7 @@ def test_vcycle_face_levels_streamed_bit_exact(mgmod, uniform, n, bc, nu):
 # V-cycles: every kernel-selection combination gives the oracle's iterate bit for bit
 # --------------------------------------------------------------------------- #
 OPTS = [dict(kernels=k, graph=gr, coarse_cta=c) for k, gr, c in itertools.product((0, 1), (0, 1), (0, 1))]
-OPTS += [dict(kernels=2, graph=1, coarse_cta=1), dict(kernels=1, graph=1, coarse_cta=1, tails=0),
+OPTS += [dict(kernels=1, graph=1, coarse_cta=1, tails=0),
          dict(kernels=1, graph=0, coarse_cta=1, fuse=1)]
 
 
