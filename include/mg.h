@@ -65,7 +65,8 @@ enum {
     MG_OPT_COARSE_CTA = 3,  /* 1 (default) = levels <= 16^3 run in one persistent CTA       */
     MG_OPT_SWEEP_FUSE = 4,  /* sweeps fused per pass of the TMA kernel: 1 or 2 (default) */
     MG_OPT_TAIL_FUSION = 5, /* 1 (default) = residual+restriction fused behind the last pre-sweep
-                               and, in mg_solve, sum r^2 behind the last post-sweep (level 0);
+                               and, in mg_solve, sum r^2 behind the last post-sweep, on level 0;
+                               2 = the restriction tail on the streamed stored-face levels too;
                                0 = separate passes */
     MG_OPT_FACE_STREAM_LOG2 = 6 /* stored-face levels (>= 1) with at least 2^value cells use the
                                TMA kernel, smaller ones two half-sweep launches per sweep

@@ -2,7 +2,8 @@
 
     python -m paper_2605_30082_b200.profile_driver --step sweep2 --workload config4 --reps 3
 
-steps: sweep2 (two level-0 sweeps), sweep1, vcycle, residual, solve.  Prints the average
+steps: sweep4, sweep2, sweep1 (that many sweeps on --level), sweep_restrict (one sweep with the
+residual + restriction tail), vcycle, residual, solve.  Prints the average
 CUDA-event time per repetition.  Uses only the public binding and the workload generator.
 """
 import argparse
@@ -52,6 +53,8 @@ def main():
                 g.level_smooth(args.level, 2, f, p)
             elif args.step == "sweep1":
                 g.level_smooth(args.level, 1, f, p)
+            elif args.step == "sweep_restrict":
+                g.level_smooth_restrict(args.level, 1, f, p)
             elif args.step == "vcycle":
                 g.vcycle(f, p)
             elif args.step == "residual":

@@ -199,7 +199,7 @@ FACE_SHAPES = [
 @pytest.mark.parametrize("fuse", [1, 2])
 def test_face_levels_streamed_bit_exact(mgmod, uniform, n, bc, fuse):
     shp = (n[2], n[1], n[0])
-    o, g = pair(mgmod, n, 1.0 / n[0], bc, rho=random_rho(uniform, 61, shp), fuse=fuse, face_log2=0)
+    o, g = pair(mgmod, n, 1.0 / n[0], bc, rho=random_rho(uniform, 61, shp), fuse=fuse, face_log2=0, tails=2)
     for lvl in range(1, o.num_levels - 1):
         lshp = o.level_shape(lvl)                      # (nz, ny, nx)
         if min(lshp[1], lshp[2]) < 32 or lshp[0] < 16:
@@ -223,9 +223,11 @@ def test_face_levels_streamed_bit_exact(mgmod, uniform, n, bc, fuse):
 
 @pytest.mark.parametrize("n,bc", FACE_SHAPES)
 @pytest.mark.parametrize("nu", [(2, 2), (3, 3)])
-def test_vcycle_face_levels_streamed_bit_exact(mgmod, uniform, n, bc, nu):
+@pytest.mark.parametrize("tails", [1, 2])
+def test_vcycle_face_levels_streamed_bit_exact(mgmod, uniform, n, bc, nu, tails):
     shp = (n[2], n[1], n[0])
-    o, g = pair(mgmod, n, 1.0 / n[0], bc, nu=nu, rho=random_rho(uniform, 71, shp), coarse_sweeps=8, face_log2=0)
+    o, g = pair(mgmod, n, 1.0 / n[0], bc, nu=nu, rho=random_rho(uniform, 71, shp), coarse_sweeps=8, face_log2=0,
+                tails=tails)
     f = uniform(72, shp)
     f -= f.mean()
     po, pg, fd = np.zeros(shp), dev(np.zeros(shp)), dev(f)
