@@ -23,13 +23,17 @@ typedef struct {
     int nx, ny, nz;
     double h, h2, ih2;          /* C1 */
     double *bx, *by, *bz;       /* minus-face coefficients */
+    double *wx, *wy, *wz;       /* R24: plus-wall face coefficients of a non-periodic axis:
+                                 * wx[j + ny*k] belongs to cell (nx-1, j, k), wy[i + nx*k], wz[i + nx*j] */
+    int walled[3];              /* axis is not periodic: walls at both ends (R24) */
     double *p, *f;              /* levels >= 1: correction e and restricted rhs */
     double *r;                  /* residual scratch (levels that have a coarser one) */
 } level_t;
 
 struct mgo_solver {
     int nlev;
-    int bc[3];
+    int bc[3];                  /* per axis, as given to mgo_create (both sides alike) */
+    int bcm[3], bcp[3];         /* R24: per side (minus, plus): MGO_BC_PERIODIC / NEUMANN / DIRICHLET */
     int nu1, nu2, coarse_sweeps;
     int cycle_type;             /* R23: MGO_CYCLE_V / F / W */
     level_t lv[MGO_MAX_LEVELS];
@@ -63,14 +67,31 @@ int mgo_create(int nx, int ny, int nz, double h, const int bc[3], mgo_solver **o
 {
     if (!out || !bc) return MGO_EINVAL;
     *out = NULL;
-    if (nx < 4 || ny < 4 || nz < 4 || (nx & 1) || (ny & 1) || (nz & 1)) return MGO_EINVAL;
-    if (!(h > 0.0) || !isfinite(h)) return MGO_EINVAL;
     for (int a = 0; a < 3; ++a)
         if (bc[a] != 0 && bc[a] != 1) return MGO_EINVAL;
+    const int bc6[6] = { bc[0], bc[0], bc[1], bc[1], bc[2], bc[2] };
+    return mgo_create6(nx, ny, nz, h, bc6, out);
+}
+
+/* R24: one boundary type per side, order x-, x+, y-, y+, z-, z+.  Periodic comes in pairs. */
+int mgo_create6(int nx, int ny, int nz, double h, const int bc6[6], mgo_solver **out)
+{
+    if (!out || !bc6) return MGO_EINVAL;
+    *out = NULL;
+    if (nx < 4 || ny < 4 || nz < 4 || (nx & 1) || (ny & 1) || (nz & 1)) return MGO_EINVAL;
+    if (!(h > 0.0) || !isfinite(h)) return MGO_EINVAL;
+    for (int a = 0; a < 3; ++a) {
+        const int m = bc6[2 * a], q = bc6[2 * a + 1];
+        if (m < MGO_BC_PERIODIC || m > MGO_BC_DIRICHLET || q < MGO_BC_PERIODIC || q > MGO_BC_DIRICHLET) return MGO_EINVAL;
+        if ((m == MGO_BC_PERIODIC) != (q == MGO_BC_PERIODIC)) return MGO_EINVAL;
+    }
 
     mgo_solver *s = (mgo_solver *)calloc(1, sizeof(*s));
     if (!s) return MGO_ENOMEM;
-    memcpy(s->bc, bc, sizeof(s->bc));
+    for (int a = 0; a < 3; ++a) {
+        s->bcm[a] = bc6[2 * a]; s->bcp[a] = bc6[2 * a + 1];
+        s->bc[a] = s->bcm[a] == MGO_BC_PERIODIC ? 0 : 1;
+    }
     s->nu1 = 2; s->nu2 = 2; s->coarse_sweeps = 32;
 
     /* R7: halve every axis while the halved dims stay even (so red-black colouring is
@@ -82,6 +103,7 @@ int mgo_create(int nx, int ny, int nz, double h, const int bc[3], mgo_solver **o
         level_t *L = &s->lv[l];
         L->nx = n[0]; L->ny = n[1]; L->nz = n[2];
         L->h = hl; L->h2 = hl * hl; L->ih2 = 1.0 / L->h2;
+        for (int a = 0; a < 3; ++a) L->walled[a] = s->bcm[a] != MGO_BC_PERIODIC;
         ++l;
         int mn = n[0] < n[1] ? n[0] : n[1]; if (n[2] < mn) mn = n[2];
         if (mn <= 4 || (n[0] % 4) || (n[1] % 4) || (n[2] % 4) || l == MGO_MAX_LEVELS) break;
@@ -94,12 +116,15 @@ int mgo_create(int nx, int ny, int nz, double h, const int bc[3], mgo_solver **o
         L->bx = (double *)malloc(N * sizeof(double));
         L->by = (double *)malloc(N * sizeof(double));
         L->bz = (double *)malloc(N * sizeof(double));
+        L->wx = (double *)calloc((size_t)L->ny * L->nz, sizeof(double));
+        L->wy = (double *)calloc((size_t)L->nx * L->nz, sizeof(double));
+        L->wz = (double *)calloc((size_t)L->nx * L->ny, sizeof(double));
         if (l > 0) {
             L->p = (double *)malloc(N * sizeof(double));
             L->f = (double *)malloc(N * sizeof(double));
         }
         if (l < s->nlev - 1) L->r = (double *)malloc(N * sizeof(double));
-        if (!L->bx || !L->by || !L->bz || (l > 0 && (!L->p || !L->f)) ||
+        if (!L->bx || !L->by || !L->bz || !L->wx || !L->wy || !L->wz || (l > 0 && (!L->p || !L->f)) ||
             (l < s->nlev - 1 && !L->r)) { mgo_destroy(s); return MGO_ENOMEM; }
     }
     /* default density rho == 1 */
@@ -121,6 +146,7 @@ void mgo_destroy(mgo_solver *s)
     if (!s) return;
     for (int l = 0; l < s->nlev; ++l) {
         free(s->lv[l].bx); free(s->lv[l].by); free(s->lv[l].bz);
+        free(s->lv[l].wx); free(s->lv[l].wy); free(s->lv[l].wz);
         free(s->lv[l].p); free(s->lv[l].f); free(s->lv[l].r);
     }
     free(s);
@@ -144,7 +170,9 @@ int mgo_set_density(mgo_solver *s, const double *rho)
         if (!(rho[c] > 0.0) || !isfinite(rho[c])) return MGO_EINVAL;
 
     /* C2: a = 0.5/rho per cell; face between cells c and nb: beta = a[c] + a[nb];
-     * Neumann wall face: beta = +0.0.  (R4: beta = 1/rho_face, rho_face harmonic mean) */
+     * Neumann wall face: beta = +0.0.  (R4: beta = 1/rho_face, rho_face harmonic mean)
+     * R24 / C2w: Dirichlet wall face (p = 0 ON the face, ghost = -p_c, ghost density = the cell's):
+     * beta_w (0 - p_c) with beta_w = 2.0 * (a[c] + a[c]). */
     double *a = (double *)malloc(N * sizeof(double));
     if (!a) return MGO_ENOMEM;
     for (size_t c = 0; c < N; ++c) a[c] = 0.5 / rho[c];
@@ -156,9 +184,16 @@ int mgo_set_density(mgo_solver *s, const double *rho)
                 int im = i == 0 ? nx - 1 : i - 1;
                 int jm = j == 0 ? ny - 1 : j - 1;
                 int km = k == 0 ? nz - 1 : k - 1;
-                L->bx[c] = (s->bc[0] == 1 && i == 0) ? 0.0 : a[c] + a[IDX(L, im, j, k)];
-                L->by[c] = (s->bc[1] == 1 && j == 0) ? 0.0 : a[c] + a[IDX(L, i, jm, k)];
-                L->bz[c] = (s->bc[2] == 1 && k == 0) ? 0.0 : a[c] + a[IDX(L, i, j, km)];
+                const double wall = 2.0 * (a[c] + a[c]);
+                L->bx[c] = (i == 0 && s->bcm[0] != MGO_BC_PERIODIC) ? (s->bcm[0] == MGO_BC_DIRICHLET ? wall : 0.0)
+                                                                    : a[c] + a[IDX(L, im, j, k)];
+                L->by[c] = (j == 0 && s->bcm[1] != MGO_BC_PERIODIC) ? (s->bcm[1] == MGO_BC_DIRICHLET ? wall : 0.0)
+                                                                    : a[c] + a[IDX(L, i, jm, k)];
+                L->bz[c] = (k == 0 && s->bcm[2] != MGO_BC_PERIODIC) ? (s->bcm[2] == MGO_BC_DIRICHLET ? wall : 0.0)
+                                                                    : a[c] + a[IDX(L, i, j, km)];
+                if (i == nx - 1) L->wx[j + (size_t)ny * k] = s->bcp[0] == MGO_BC_DIRICHLET ? wall : 0.0;
+                if (j == ny - 1) L->wy[i + (size_t)nx * k] = s->bcp[1] == MGO_BC_DIRICHLET ? wall : 0.0;
+                if (k == nz - 1) L->wz[i + (size_t)nx * j] = s->bcp[2] == MGO_BC_DIRICHLET ? wall : 0.0;
             }
     free(a);
 
@@ -179,12 +214,34 @@ int mgo_set_density(mgo_solver *s, const double *rho)
                     C->bz[c] = 0.25 * ((F->bz[IDX(F, i, j, k)] + F->bz[IDX(F, i + 1, j, k)]) +
                                        (F->bz[IDX(F, i, j + 1, k)] + F->bz[IDX(F, i + 1, j + 1, k)]));
                 }
+        /* the plus walls coarsen by the same rule (the four finer wall faces on the coarse one) */
+        for (int K = 0; K < C->nz; ++K)
+            for (int J = 0; J < C->ny; ++J) {
+                const size_t m = F->ny;
+                C->wx[J + (size_t)C->ny * K] = 0.25 * ((F->wx[2 * J + m * (2 * K)] + F->wx[2 * J + 1 + m * (2 * K)]) +
+                                                       (F->wx[2 * J + m * (2 * K + 1)] + F->wx[2 * J + 1 + m * (2 * K + 1)]));
+            }
+        for (int K = 0; K < C->nz; ++K)
+            for (int I = 0; I < C->nx; ++I) {
+                const size_t m = F->nx;
+                C->wy[I + (size_t)C->nx * K] = 0.25 * ((F->wy[2 * I + m * (2 * K)] + F->wy[2 * I + 1 + m * (2 * K)]) +
+                                                       (F->wy[2 * I + m * (2 * K + 1)] + F->wy[2 * I + 1 + m * (2 * K + 1)]));
+            }
+        for (int J = 0; J < C->ny; ++J)
+            for (int I = 0; I < C->nx; ++I) {
+                const size_t m = F->nx;
+                C->wz[I + (size_t)C->nx * J] = 0.25 * ((F->wz[2 * I + m * (2 * J)] + F->wz[2 * I + 1 + m * (2 * J)]) +
+                                                       (F->wz[2 * I + m * (2 * J + 1)] + F->wz[2 * I + 1 + m * (2 * J + 1)]));
+            }
     }
     return MGO_OK;
 }
 
 /* ------------------------------------------------------------- the stencil */
-/* C4: neighbour sum S and diagonal D of cell (i,j,k), order x-,x+,y-,y+,z-,z+ */
+/* C4: neighbour sum S and diagonal D of cell (i,j,k), order x-,x+,y-,y+,z-,z+.
+ * At a wall (non-periodic axis, R5 / R24) the face coefficient is the stored wall value (minus
+ * wall: entry 0 of the minus-face array; plus wall: wx / wy / wz) and the neighbour value is 0.0
+ * (C2: Neumann wall 0.0 * 0.0; Dirichlet wall beta_w * 0.0 with beta_w in D). */
 static inline void stencil(const level_t *L, const double *p, int i, int j, int k,
                            double *S, double *D)
 {
@@ -192,12 +249,15 @@ static inline void stencil(const level_t *L, const double *p, int i, int j, int 
     const int im = i == 0 ? nx - 1 : i - 1, ip = i == nx - 1 ? 0 : i + 1;
     const int jm = j == 0 ? ny - 1 : j - 1, jp = j == ny - 1 ? 0 : j + 1;
     const int km = k == 0 ? nz - 1 : k - 1, kp = k == nz - 1 ? 0 : k + 1;
-    const double bxm = L->bx[IDX(L, i, j, k)], bxp = L->bx[IDX(L, ip, j, k)];
-    const double bym = L->by[IDX(L, i, j, k)], byp = L->by[IDX(L, i, jp, k)];
-    const double bzm = L->bz[IDX(L, i, j, k)], bzp = L->bz[IDX(L, i, j, kp)];
-    const double pxm = p[IDX(L, im, j, k)], pxp = p[IDX(L, ip, j, k)];
-    const double pym = p[IDX(L, i, jm, k)], pyp = p[IDX(L, i, jp, k)];
-    const double pzm = p[IDX(L, i, j, km)], pzp = p[IDX(L, i, j, kp)];
+    const int wxm = L->walled[0] && i == 0, wxp = L->walled[0] && i == nx - 1;
+    const int wym = L->walled[1] && j == 0, wyp = L->walled[1] && j == ny - 1;
+    const int wzm = L->walled[2] && k == 0, wzp = L->walled[2] && k == nz - 1;
+    const double bxm = L->bx[IDX(L, i, j, k)], bxp = wxp ? L->wx[j + (size_t)ny * k] : L->bx[IDX(L, ip, j, k)];
+    const double bym = L->by[IDX(L, i, j, k)], byp = wyp ? L->wy[i + (size_t)nx * k] : L->by[IDX(L, i, jp, k)];
+    const double bzm = L->bz[IDX(L, i, j, k)], bzp = wzp ? L->wz[i + (size_t)nx * j] : L->bz[IDX(L, i, j, kp)];
+    const double pxm = wxm ? 0.0 : p[IDX(L, im, j, k)], pxp = wxp ? 0.0 : p[IDX(L, ip, j, k)];
+    const double pym = wym ? 0.0 : p[IDX(L, i, jm, k)], pyp = wyp ? 0.0 : p[IDX(L, i, jp, k)];
+    const double pzm = wzm ? 0.0 : p[IDX(L, i, j, km)], pzp = wzp ? 0.0 : p[IDX(L, i, j, kp)];
     *S = fma(bzp, pzp, fma(bzm, pzm, fma(byp, pyp, fma(bym, pym, fma(bxp, pxp, bxm * pxm)))));
     *D = ((((bxm + bxp) + bym) + byp) + bzm) + bzp;
 }
@@ -267,16 +327,26 @@ static void restrict8(const level_t *F, const level_t *C, const double *r, doubl
 
 static inline double lerp(double near, double far) { return fma(0.25, far, 0.75 * near); }
 
-/* neighbour coarse index on the side the fine child leans to; wrap, or clamp (Neumann) */
-static inline int far_index(int I, int side, int n, int neumann)
+/* neighbour coarse index on the side the fine child leans to: wrap (periodic), the boundary cell
+ * itself beyond a wall.  *sign = -1.0 beyond a Dirichlet wall (R24: ghost = -e_boundary, so that
+ * the interpolant vanishes on the wall), +1.0 otherwise (Neumann: ghost = e_boundary, R12). */
+static inline int far_index(int I, int side, int n, int bc_minus, int bc_plus, double *sign)
 {
     int Ip = I + 2 * side - 1;
-    if (Ip < 0) Ip = neumann ? 0 : n - 1;
-    if (Ip >= n) Ip = neumann ? n - 1 : 0;
+    *sign = 1.0;
+    if (Ip < 0) {
+        if (bc_minus == MGO_BC_PERIODIC) Ip = n - 1;
+        else { Ip = 0; if (bc_minus == MGO_BC_DIRICHLET) *sign = -1.0; }
+    }
+    if (Ip >= n) {
+        if (bc_plus == MGO_BC_PERIODIC) Ip = 0;
+        else { Ip = n - 1; if (bc_plus == MGO_BC_DIRICHLET) *sign = -1.0; }
+    }
     return Ip;
 }
 
-/* C8 (R12): p += cell-centred trilinear interpolation of e (x first, then y, then z) */
+/* C8 (R12): p += cell-centred trilinear interpolation of e (x first, then y, then z); a value
+ * taken beyond Dirichlet walls carries the product of the signs of those axes */
 static void prolong_add(const mgo_solver *s, const level_t *F, const level_t *C,
                         const double *e, double *p)
 {
@@ -285,14 +355,15 @@ static void prolong_add(const mgo_solver *s, const level_t *F, const level_t *C,
         for (int j = 0; j < F->ny; ++j)
             for (int i = 0; i < F->nx; ++i) {
                 const int I = i >> 1, J = j >> 1, K = k >> 1;
-                const int Ip = far_index(I, i & 1, C->nx, s->bc[0] == 1);
-                const int Jp = far_index(J, j & 1, C->ny, s->bc[1] == 1);
-                const int Kp = far_index(K, k & 1, C->nz, s->bc[2] == 1);
+                double sx, sy, sz;
+                const int Ip = far_index(I, i & 1, C->nx, s->bcm[0], s->bcp[0], &sx);
+                const int Jp = far_index(J, j & 1, C->ny, s->bcm[1], s->bcp[1], &sy);
+                const int Kp = far_index(K, k & 1, C->nz, s->bcm[2], s->bcp[2], &sz);
                 const double v =
-                    lerp(lerp(lerp(e[IDX(C, I, J, K)],   e[IDX(C, Ip, J, K)]),
-                              lerp(e[IDX(C, I, Jp, K)],  e[IDX(C, Ip, Jp, K)])),
-                         lerp(lerp(e[IDX(C, I, J, Kp)],  e[IDX(C, Ip, J, Kp)]),
-                              lerp(e[IDX(C, I, Jp, Kp)], e[IDX(C, Ip, Jp, Kp)])));
+                    lerp(lerp(lerp(e[IDX(C, I, J, K)],             sx * e[IDX(C, Ip, J, K)]),
+                              lerp(sy * e[IDX(C, I, Jp, K)],       (sx * sy) * e[IDX(C, Ip, Jp, K)])),
+                         lerp(lerp(sz * e[IDX(C, I, J, Kp)],       (sx * sz) * e[IDX(C, Ip, J, Kp)]),
+                              lerp((sy * sz) * e[IDX(C, I, Jp, Kp)], ((sx * sy) * sz) * e[IDX(C, Ip, Jp, Kp)])));
                 p[IDX(F, i, j, k)] = p[IDX(F, i, j, k)] + v;
             }
 }
@@ -314,6 +385,14 @@ static long double sum_planes(const level_t *L, const double *x, int squared)
     for (int k = 0; k < L->nz; ++k) tot += part[k];
     free(part);
     return tot;
+}
+
+/* R6 / R24: the operator is singular (null space = constants) unless some side is a Dirichlet wall */
+static int has_dirichlet(const mgo_solver *s)
+{
+    for (int a = 0; a < 3; ++a)
+        if (s->bcm[a] == MGO_BC_DIRICHLET || s->bcp[a] == MGO_BC_DIRICHLET) return 1;
+    return 0;
 }
 
 /* ------------------------------------------------------------------ cycle */
@@ -388,7 +467,8 @@ int mgo_solve(mgo_solver *s, const double *rhs, double *p, double rtol, int max_
     level_t *L = &s->lv[0];
     const size_t N = lv_cells(L);
     /* R6: singular system (all axes periodic/Neumann): the rhs must be mean-free */
-    {
+    const int singular = !has_dirichlet(s);
+    if (singular) {
         long double mean = sum_planes(L, rhs, 0) / (long double)N;
         long double nrm = sqrtl(sum_planes(L, rhs, 1));
         if (fabsl(mean) > 1e-12L * (nrm / sqrtl((long double)N))) return MGO_EINCOMPATIBLE;
@@ -407,8 +487,8 @@ int mgo_solve(mgo_solver *s, const double *rhs, double *p, double rtol, int max_
         if (!isfinite(rk)) { if (cycles_out) *cycles_out = k; return MGO_EDIVERGED; }
         if (rk <= rtol * r0) status = MGO_OK;
     }
-    /* zero arithmetic mean, once, at the end (R6) */
-    {
+    /* zero arithmetic mean, once, at the end (R6); with a Dirichlet wall p is unique as it is */
+    if (singular) {
         double mean = (double)(sum_planes(L, p, 0) / (long double)N);
         for (size_t c = 0; c < N; ++c) p[c] = p[c] - mean;
     }
@@ -446,7 +526,8 @@ static void sweep_rev(const level_t *L, const double *f, double *p)
 static inline double pt_weight(int i, int I, int cn, int neumann)
 {
     const int near = i >> 1;
-    const int far = far_index(near, i & 1, cn, neumann);
+    double sign;            /* (periodic or Neumann sides only here: the sign is always +1) */
+    const int far = far_index(near, i & 1, cn, neumann, neumann, &sign);
     return (near == I ? 0.75 : 0.0) + (far == I ? 0.25 : 0.0);
 }
 
@@ -511,7 +592,7 @@ static void vcycle_sym(mgo_solver *s, int l, double *p, const double *f)
 
 int mgo_restrict_adj(const mgo_solver *s, int level, const double *r, double *fc)
 {
-    if (!s || level < 0 || level >= s->nlev - 1 || !r || !fc) return MGO_EINVAL;
+    if (!s || level < 0 || level >= s->nlev - 1 || !r || !fc || has_dirichlet(s)) return MGO_EINVAL;
     restrict_adj(s, &s->lv[level], &s->lv[level + 1], r, fc);
     return MGO_OK;
 }
@@ -519,7 +600,7 @@ int mgo_restrict_adj(const mgo_solver *s, int level, const double *r, double *fc
 /* z = M r: one symmetric cycle from z = 0 */
 int mgo_precondition(mgo_solver *s, const double *r, double *z)
 {
-    if (!s || !r || !z || s->nu1 != s->nu2) return MGO_EINVAL;
+    if (!s || !r || !z || s->nu1 != s->nu2 || has_dirichlet(s)) return MGO_EINVAL;
     memset(z, 0, lv_cells(&s->lv[0]) * sizeof(double));
     vcycle_sym(s, 0, z, r);
     return MGO_OK;
@@ -545,7 +626,7 @@ static long double dot_planes(const level_t *L, const double *x, const double *y
 int mgo_solve_pcg(mgo_solver *s, const double *rhs, double *p, double rtol, int max_iter,
                   int *iters_out, double *relres_out, double *hist)
 {
-    if (!s || !rhs || !p || !(rtol >= 0.0) || max_iter < 0 || s->nu1 != s->nu2) return MGO_EINVAL;
+    if (!s || !rhs || !p || !(rtol >= 0.0) || max_iter < 0 || s->nu1 != s->nu2 || has_dirichlet(s)) return MGO_EINVAL;
     level_t *L = &s->lv[0];
     const size_t N = lv_cells(L);
     {
@@ -620,7 +701,7 @@ int mgo_solve_pcg(mgo_solver *s, const double *rhs, double *p, double rtol, int 
 int mgo_project_rhs(const mgo_solver *s, const double *u, const double *v, const double *w,
                     double dt, double *f)
 {
-    if (!s || !u || !v || !w || !f || !(dt > 0.0) || !isfinite(dt)) return MGO_EINVAL;
+    if (!s || !u || !v || !w || !f || !(dt > 0.0) || !isfinite(dt) || has_dirichlet(s)) return MGO_EINVAL;
     const level_t *L = &s->lv[0];
     const int nx = L->nx, ny = L->ny, nz = L->nz;
     const double hd = L->h * dt;
@@ -643,7 +724,7 @@ int mgo_project_rhs(const mgo_solver *s, const double *u, const double *v, const
 
 int mgo_project_correct(const mgo_solver *s, const double *p, double dt, double *u, double *v, double *w)
 {
-    if (!s || !u || !v || !w || !p || !(dt > 0.0) || !isfinite(dt)) return MGO_EINVAL;
+    if (!s || !u || !v || !w || !p || !(dt > 0.0) || !isfinite(dt) || has_dirichlet(s)) return MGO_EINVAL;
     const level_t *L = &s->lv[0];
     const int nx = L->nx, ny = L->ny, nz = L->nz;
     const double g = dt / L->h;
@@ -671,6 +752,16 @@ int mgo_level_dims(const mgo_solver *s, int level, int dims[3], double *h_level)
     if (!s || level < 0 || level >= s->nlev) return MGO_EINVAL;
     if (dims) { dims[0] = s->lv[level].nx; dims[1] = s->lv[level].ny; dims[2] = s->lv[level].nz; }
     if (h_level) *h_level = s->lv[level].h;
+    return MGO_OK;
+}
+
+int mgo_get_walls(const mgo_solver *s, int level, double *wx, double *wy, double *wz)
+{
+    if (!s || level < 0 || level >= s->nlev) return MGO_EINVAL;
+    const level_t *L = &s->lv[level];
+    if (wx) memcpy(wx, L->wx, (size_t)L->ny * L->nz * sizeof(double));
+    if (wy) memcpy(wy, L->wy, (size_t)L->nx * L->nz * sizeof(double));
+    if (wz) memcpy(wz, L->wz, (size_t)L->nx * L->ny * sizeof(double));
     return MGO_OK;
 }
 

@@ -51,6 +51,17 @@ enum { MGO_OK = 0, MGO_NOT_CONVERGED = 1, MGO_EINVAL = -1, MGO_ENOMEM = -2,
 
 /* bc[axis]: 0 periodic, 1 homogeneous Neumann.  Density defaults to rho == 1. */
 int  mgo_create(int nx, int ny, int nz, double h, const int bc[3], mgo_solver **out);
+/* R24 (the paper's box has a no-slip base, two symmetry planes and "continuous"
+ * outflow planes): one boundary type per side, order x-, x+, y-, y+, z-, z+.
+ * PERIODIC must be given for both sides of an axis.  NEUMANN: no flux through the wall (face
+ * coefficient 0).  DIRICHLET: p = 0 on the wall face: the ghost value is -p_c, ghost density the
+ * cell's, i.e. a wall face of coefficient 2 (a_c + a_c) whose neighbour value is 0; coarse walls
+ * are the mean of the four finer wall faces (C3); the prolongation ghost is -e_boundary.  With a
+ * Dirichlet wall the system is non-singular: mgo_solve checks no compatibility and removes no
+ * mean.  mgo_solve_pcg / mgo_precondition / mgo_restrict_adj / mgo_project_* return MGO_EINVAL
+ * on such a solver (they are defined for periodic and Neumann sides). */
+enum { MGO_BC_PERIODIC = 0, MGO_BC_NEUMANN = 1, MGO_BC_DIRICHLET = 2 };
+int  mgo_create6(int nx, int ny, int nz, double h, const int bc6[6], mgo_solver **out);
 void mgo_destroy(mgo_solver *s);
 int  mgo_set_cycle(mgo_solver *s, int nu1, int nu2, int coarse_sweeps);
 /* R23: cycle index.  V (default): one visit of the coarse problem per level;
@@ -88,6 +99,8 @@ int  mgo_project_correct(const mgo_solver *s, const double *p, double dt, double
 int  mgo_num_levels(const mgo_solver *s);
 int  mgo_level_dims(const mgo_solver *s, int level, int dims[3], double *h_level);
 /* copies the minus-face coefficient arrays of `level` (each nx*ny*nz of that level) */
+/* plus-wall face coefficients of level `level`: wx[ny*nz], wy[nx*nz], wz[nx*ny] (0 on a periodic axis) */
+int  mgo_get_walls(const mgo_solver *s, int level, double *wx, double *wy, double *wz);
 int  mgo_get_faces(const mgo_solver *s, int level, double *bx, double *by, double *bz);
 /* out = A_level p */
 int  mgo_apply(const mgo_solver *s, int level, const double *p, double *out);

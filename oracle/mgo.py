@@ -62,7 +62,9 @@ def lib():
         ip = C.POINTER(C.c_int)
         vp = C.c_void_p
         L.mgo_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, ip, C.POINTER(vp)]
+        L.mgo_create6.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, ip, C.POINTER(vp)]
         L.mgo_destroy.argtypes = [vp]
+        L.mgo_get_walls.argtypes = [vp, C.c_int, dp, dp, dp]
         L.mgo_destroy.restype = None
         L.mgo_set_cycle.argtypes = [vp, C.c_int, C.c_int, C.c_int]
         L.mgo_set_cycle_type.argtypes = [vp, C.c_int]
@@ -116,8 +118,12 @@ class Oracle:
         self.h = float(h)
         self.bc = tuple(int(b) for b in bc)
         self._h = C.c_void_p()
-        bca = (C.c_int * 3)(*self.bc)
-        _chk(lib().mgo_create(self.n[0], self.n[1], self.n[2], self.h, bca, C.byref(self._h)))
+        if len(self.bc) == 6:           # R24: one type per side (x-, x+, y-, y+, z-, z+); 2 = Dirichlet
+            bca = (C.c_int * 6)(*self.bc)
+            _chk(lib().mgo_create6(self.n[0], self.n[1], self.n[2], self.h, bca, C.byref(self._h)))
+        else:
+            bca = (C.c_int * 3)(*self.bc)
+            _chk(lib().mgo_create(self.n[0], self.n[1], self.n[2], self.h, bca, C.byref(self._h)))
         _chk(lib().mgo_set_cycle(self._h, nu1, nu2, coarse_sweeps))
 
     def close(self):
@@ -204,6 +210,13 @@ class Oracle:
         z = np.empty(self.shape)
         _chk(lib().mgo_precondition(self._h, _dp(self._arr(r)), _dp(z)))
         return z
+
+    def walls(self, level=0):
+        """Plus-wall face coefficients (wx[nz, ny], wy[nz, nx], wz[ny, nx]) of a level."""
+        nz, ny, nx = self.level_shape(level)
+        wx, wy, wz = np.empty((nz, ny)), np.empty((nz, nx)), np.empty((ny, nx))
+        _chk(lib().mgo_get_walls(self._h, level, _dp(wx), _dp(wy), _dp(wz)))
+        return wx, wy, wz
 
     def restrict_adj(self, r, level=0):
         fc = np.empty(self.level_shape(level + 1))
