@@ -55,7 +55,7 @@ enum {
     MG_EDIVERGED = -5       /* a residual norm became non-finite                           */
 };
 
-enum { MG_BC_PERIODIC = 0, MG_BC_NEUMANN = 1 };
+enum { MG_BC_PERIODIC = 0, MG_BC_NEUMANN = 1, MG_BC_DIRICHLET = 2 /* mg_create6 only */ };
 
 /* mg_set_option keys */
 enum {
@@ -96,6 +96,20 @@ int mg_create(int nx, int ny, int nz, double h, const int bc[3], mg_handle **out
  * keeps ownership and must keep it alive until mg_destroy. */
 int mg_create_in(int nx, int ny, int nz, double h, const int bc[3],
                  void *workspace_dev, size_t workspace_bytes, mg_handle **out);
+
+/* One boundary type per SIDE (R24; the paper's box has a no-slip
+ * base, two symmetry planes and "continuous" outflow planes): bc6 = {x-, x+, y-, y+,
+ * z-, z+}, each MG_BC_PERIODIC (both sides of the axis), MG_BC_NEUMANN (no flux through the wall)
+ * or MG_BC_DIRICHLET (p = 0 on the wall face: ghost value -p_c, i.e. a wall face of coefficient
+ * 2 (a_c + a_c) whose neighbour value is 0; coarse walls are the mean of the four finer wall
+ * faces; the prolongation ghost is -e_boundary).  With a Dirichlet wall the system is
+ * non-singular: mg_solve checks no compatibility and removes no mean.  Such a solver runs the
+ * level-generic kernels (MG_OPT_KERNELS = 0, MG_OPT_COARSE_CTA = 0; switching them on returns
+ * MG_EINVAL), and mg_project* return MG_EINVAL (the staggered velocity layout has no plus-wall
+ * face).  Without a Dirichlet side this is mg_create / mg_create_in.  Errors as mg_create. */
+int mg_create6(int nx, int ny, int nz, double h, const int bc6[6], mg_handle **out);
+int mg_create6_in(int nx, int ny, int nz, double h, const int bc6[6],
+                  void *workspace_dev, size_t workspace_bytes, mg_handle **out);
 
 /* Frees everything the library allocated (never caller buffers).  NULL is allowed. */
 void mg_destroy(mg_handle *s);

@@ -25,6 +25,8 @@ SIGNATURES = {
     "mg_workspace_bytes": (C.c_size_t, [C.c_int, C.c_int, C.c_int]),
     "mg_create": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_double, _ip, C.POINTER(_vp)]),
     "mg_create_in": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_double, _ip, _vp, C.c_size_t, C.POINTER(_vp)]),
+    "mg_create6": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_double, _ip, C.POINTER(_vp)]),
+    "mg_create6_in": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_double, _ip, _vp, C.c_size_t, C.POINTER(_vp)]),
     "mg_destroy": (None, [_vp]),
     "mg_set_stream": (C.c_int, [_vp, _vp]),
     "mg_set_cycle_type": (C.c_int, [_vp, C.c_int]),
@@ -104,7 +106,8 @@ def _ptr(t, shape=None):
 
 class Multigrid:
     """Handle to one solver.  n = (nx, ny, nz) or a single int; bc per axis (0 periodic,
-    1 Neumann).  Device storage comes from a torch tensor (mg_create_in); the stream is
+    1 Neumann), or six entries, one per side x-, x+, y-, y+, z-, z+ (2 = Dirichlet: mg_create6).
+    Device storage comes from a torch tensor (mg_create_in); the stream is
     torch's current stream at construction unless ``stream`` is given."""
 
     def __init__(self, n, h, bc, nu1=2, nu2=2, coarse_sweeps=32, stream=None, device="cuda:0",
@@ -121,14 +124,16 @@ class Multigrid:
         if need == 0:
             raise MgError(MG_EINVAL)
         with torch.cuda.device(self.device):
-            bca = (C.c_int * 3)(*[int(b) for b in bc])
+            bc = [int(b) for b in bc]
+            bca = (C.c_int * len(bc))(*bc)
+            create, create_in = (L.mg_create6, L.mg_create6_in) if len(bc) == 6 else (L.mg_create, L.mg_create_in)
             if own_workspace:           # mg_create: the library allocates with cudaMalloc
                 self._ws = None
-                _chk(L.mg_create(*self.n, float(h), bca, C.byref(self._h)))
+                _chk(create(*self.n, float(h), bca, C.byref(self._h)))
             else:
                 self._ws = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
                 base = (self._ws.data_ptr() + 255) // 256 * 256
-                _chk(L.mg_create_in(*self.n, float(h), bca, base, need, C.byref(self._h)))
+                _chk(create_in(*self.n, float(h), bca, base, need, C.byref(self._h)))
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             _chk(L.mg_set_stream(self._h, self.stream.cuda_stream))
         _chk(L.mg_set_cycle(self._h, nu1, nu2, coarse_sweeps))

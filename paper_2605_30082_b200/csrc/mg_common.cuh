@@ -19,7 +19,18 @@ struct Lv {
     double h2, ih2;             // C1: h_l^2 and 1/h_l^2
     const double *a;            // level 0: a = 0.5/rho per cell (faces formed on the fly, C2)
     const double *bx, *by, *bz; // levels >= 1: stored minus-face coefficients (C3)
+    // R24 (mg_create6): one boundary type per side.  gen != 0 selects the wall logic of the
+    // level-generic kernels: wall face = stored wall value, neighbour value 0.0.
+    int gen;
+    int bcm[3], bcp[3];         // MG_BC_* of the minus / plus side of x, y, z
+    const double *wx, *wy, *wz; // levels >= 1: plus-wall face coefficients (wx[j + ny*k], wy[i + nx*k], wz[i + nx*j])
 };
+
+// C2w: Dirichlet wall face of a cell with coefficient a (ghost = -p_c, ghost density the cell's)
+__device__ __forceinline__ double wall_face(int bc_side, double ac)
+{
+    return bc_side == 2 ? __dmul_rn(2.0, __dadd_rn(ac, ac)) : 0.0;
+}
 
 __device__ __forceinline__ size_t cidx(const Lv &L, int i, int j, int k)
 {
@@ -35,7 +46,25 @@ __device__ __forceinline__ void faces(const Lv &L, int i, int j, int k, size_t c
                                       size_t cxp, size_t cym, size_t cyp, size_t czm, size_t czp,
                                       double b[6])
 {
-    if (CELL) {
+    if (L.gen) {
+        // R24: walls of a non-periodic axis carry their own coefficient (bcx/bcy/bcz = walled)
+        if (CELL) {
+            const double ac = L.a[c];
+            b[0] = (L.bcx && i == 0) ? wall_face(L.bcm[0], ac) : __dadd_rn(ac, L.a[cxm]);
+            b[1] = (L.bcx && i == L.nx - 1) ? wall_face(L.bcp[0], ac) : __dadd_rn(ac, L.a[cxp]);
+            b[2] = (L.bcy && j == 0) ? wall_face(L.bcm[1], ac) : __dadd_rn(ac, L.a[cym]);
+            b[3] = (L.bcy && j == L.ny - 1) ? wall_face(L.bcp[1], ac) : __dadd_rn(ac, L.a[cyp]);
+            b[4] = (L.bcz && k == 0) ? wall_face(L.bcm[2], ac) : __dadd_rn(ac, L.a[czm]);
+            b[5] = (L.bcz && k == L.nz - 1) ? wall_face(L.bcp[2], ac) : __dadd_rn(ac, L.a[czp]);
+        } else {
+            b[0] = L.bx[c];
+            b[1] = (L.bcx && i == L.nx - 1) ? L.wx[(size_t)j + (size_t)L.ny * (size_t)k] : L.bx[cxp];
+            b[2] = L.by[c];
+            b[3] = (L.bcy && j == L.ny - 1) ? L.wy[(size_t)i + (size_t)L.nx * (size_t)k] : L.by[cyp];
+            b[4] = L.bz[c];
+            b[5] = (L.bcz && k == L.nz - 1) ? L.wz[(size_t)i + (size_t)L.nx * (size_t)j] : L.bz[czp];
+        }
+    } else if (CELL) {
         const double ac = L.a[c];
         b[0] = (L.bcx && i == 0) ? 0.0 : __dadd_rn(ac, L.a[cxm]);
         b[1] = (L.bcx && i == L.nx - 1) ? 0.0 : __dadd_rn(ac, L.a[cxp]);
@@ -99,7 +128,13 @@ __device__ __forceinline__ void stencil_global(const Lv &L, const double *__rest
     const size_t czm = cidx(L, i, j, km), czp = cidx(L, i, j, kp);
     double b[6];
     faces<CELL>(L, i, j, k, c, cxm, cxp, cym, cyp, czm, czp, b);
-    S = stencil_S(b, p[cxm], p[cxp], p[cym], p[cyp], p[czm], p[czp]);
+    if (L.gen) {            // a wall's neighbour value is 0.0 (C2)
+        S = stencil_S(b, (L.bcx && i == 0) ? 0.0 : p[cxm], (L.bcx && i == L.nx - 1) ? 0.0 : p[cxp],
+                      (L.bcy && j == 0) ? 0.0 : p[cym], (L.bcy && j == L.ny - 1) ? 0.0 : p[cyp],
+                      (L.bcz && k == 0) ? 0.0 : p[czm], (L.bcz && k == L.nz - 1) ? 0.0 : p[czp]);
+    } else {
+        S = stencil_S(b, p[cxm], p[cxp], p[cym], p[cyp], p[czm], p[czp]);
+    }
     D = stencil_D(b);
 }
 

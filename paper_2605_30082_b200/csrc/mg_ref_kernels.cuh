@@ -37,9 +37,9 @@ __global__ void k_faces_from_cell(Lv L, double *__restrict__ bx, double *__restr
     if (i >= L.nx || j >= L.ny) return;
     const size_t c = cidx(L, i, j, k);
     const double ac = L.a[c];
-    bx[c] = (L.bcx && i == 0) ? 0.0 : __dadd_rn(ac, L.a[cidx(L, i == 0 ? L.nx - 1 : i - 1, j, k)]);
-    by[c] = (L.bcy && j == 0) ? 0.0 : __dadd_rn(ac, L.a[cidx(L, i, j == 0 ? L.ny - 1 : j - 1, k)]);
-    bz[c] = (L.bcz && k == 0) ? 0.0 : __dadd_rn(ac, L.a[cidx(L, i, j, k == 0 ? L.nz - 1 : k - 1)]);
+    bx[c] = (L.bcx && i == 0) ? wall_face(L.gen ? L.bcm[0] : 1, ac) : __dadd_rn(ac, L.a[cidx(L, i == 0 ? L.nx - 1 : i - 1, j, k)]);
+    by[c] = (L.bcy && j == 0) ? wall_face(L.gen ? L.bcm[1] : 1, ac) : __dadd_rn(ac, L.a[cidx(L, i, j == 0 ? L.ny - 1 : j - 1, k)]);
+    bz[c] = (L.bcz && k == 0) ? wall_face(L.gen ? L.bcm[2] : 1, ac) : __dadd_rn(ac, L.a[cidx(L, i, j, k == 0 ? L.nz - 1 : k - 1)]);
 }
 
 // C3: coarse minus faces = mean of the 4 finer minus faces of the even children.
@@ -50,14 +50,14 @@ __device__ __forceinline__ double fine_face(const Lv &F, int axis, int i, int j,
     const size_t c = cidx(F, i, j, k);
     if (!FINE_CELL) return axis == 0 ? F.bx[c] : (axis == 1 ? F.by[c] : F.bz[c]);
     if (axis == 0) {
-        if (F.bcx && i == 0) return 0.0;
+        if (F.bcx && i == 0) return wall_face(F.gen ? F.bcm[0] : 1, F.a[c]);
         return __dadd_rn(F.a[c], F.a[cidx(F, i == 0 ? F.nx - 1 : i - 1, j, k)]);
     }
     if (axis == 1) {
-        if (F.bcy && j == 0) return 0.0;
+        if (F.bcy && j == 0) return wall_face(F.gen ? F.bcm[1] : 1, F.a[c]);
         return __dadd_rn(F.a[c], F.a[cidx(F, i, j == 0 ? F.ny - 1 : j - 1, k)]);
     }
-    if (F.bcz && k == 0) return 0.0;
+    if (F.bcz && k == 0) return wall_face(F.gen ? F.bcm[2] : 1, F.a[c]);
     return __dadd_rn(F.a[c], F.a[cidx(F, i, j, k == 0 ? F.nz - 1 : k - 1)]);
 }
 
@@ -80,6 +80,34 @@ __global__ void k_coarsen_faces(Lv F, int cnx, int cny, int cnz, double *__restr
     cbz[c] = __dmul_rn(0.25, __dadd_rn(
         __dadd_rn(fine_face<FINE_CELL>(F, 2, i, j, k),     fine_face<FINE_CELL>(F, 2, i + 1, j, k)),
         __dadd_rn(fine_face<FINE_CELL>(F, 2, i, j + 1, k), fine_face<FINE_CELL>(F, 2, i + 1, j + 1, k))));
+}
+
+// R24: plus-wall faces of the coarse level = mean of the four finer plus-wall faces lying on
+// them, pairs in the order of C3 (over the faster in-plane axis first).  One thread per coarse
+// wall cell of one axis (blockIdx.z = axis); (u, v) = the two in-plane indices, u faster.
+template <bool FINE_CELL>
+__device__ __forceinline__ double fine_wall(const Lv &F, int axis, int u, int v)
+{
+    if (!FINE_CELL)
+        return axis == 0 ? F.wx[(size_t)u + (size_t)F.ny * (size_t)v]
+                         : (axis == 1 ? F.wy[(size_t)u + (size_t)F.nx * (size_t)v] : F.wz[(size_t)u + (size_t)F.nx * (size_t)v]);
+    const size_t c = axis == 0 ? cidx(F, F.nx - 1, u, v) : (axis == 1 ? cidx(F, u, F.ny - 1, v) : cidx(F, u, v, F.nz - 1));
+    return wall_face(F.bcp[axis], F.a[c]);
+}
+
+template <bool FINE_CELL>
+__global__ void k_coarsen_walls(Lv F, int cnx, int cny, int cnz, double *__restrict__ cwx,
+                                double *__restrict__ cwy, double *__restrict__ cwz)
+{
+    const int axis = blockIdx.z;
+    const int nu = axis == 0 ? cny : cnx, nv = axis == 2 ? cny : cnz;
+    const int U = blockIdx.x * blockDim.x + threadIdx.x, V = blockIdx.y * blockDim.y + threadIdx.y;
+    if (U >= nu || V >= nv) return;
+    const double w = __dmul_rn(0.25, __dadd_rn(
+        __dadd_rn(fine_wall<FINE_CELL>(F, axis, 2 * U, 2 * V),     fine_wall<FINE_CELL>(F, axis, 2 * U + 1, 2 * V)),
+        __dadd_rn(fine_wall<FINE_CELL>(F, axis, 2 * U, 2 * V + 1), fine_wall<FINE_CELL>(F, axis, 2 * U + 1, 2 * V + 1))));
+    double *dst = axis == 0 ? cwx : (axis == 1 ? cwy : cwz);
+    dst[(size_t)U + (size_t)nu * (size_t)V] = w;
 }
 
 // ---- A1/A6: one colour of a red-black Gauss-Seidel sweep (C4, C5) ------------
@@ -188,10 +216,40 @@ __device__ __forceinline__ int far_index(int I, int side, int n, int neumann)
     return Ip;
 }
 
+// R24: the far coarse index beyond a wall is the boundary cell itself; beyond a Dirichlet wall its
+// value enters with sign -1 (ghost = -e_boundary)
+__device__ __forceinline__ int far_index6(int I, int side, int n, int bc_minus, int bc_plus, double &sign)
+{
+    int Ip = I + 2 * side - 1;
+    sign = 1.0;
+    if (Ip < 0) {
+        if (bc_minus == 0) Ip = n - 1;
+        else { Ip = 0; if (bc_minus == 2) sign = -1.0; }
+    }
+    if (Ip >= n) {
+        if (bc_plus == 0) Ip = 0;
+        else { Ip = n - 1; if (bc_plus == 2) sign = -1.0; }
+    }
+    return Ip;
+}
+
 __device__ __forceinline__ double prolong_value(const Lv &L, const double *__restrict__ e, int cnx,
                                                 int cny, int cnz, int i, int j, int k)
 {
     const int I = i >> 1, J = j >> 1, K = k >> 1;
+    if (L.gen) {
+        double sx, sy, sz;
+        const int Ip = far_index6(I, i & 1, cnx, L.bcm[0], L.bcp[0], sx);
+        const int Jp = far_index6(J, j & 1, cny, L.bcm[1], L.bcp[1], sy);
+        const int Kp = far_index6(K, k & 1, cnz, L.bcm[2], L.bcp[2], sz);
+        const double sxy = __dmul_rn(sx, sy), sxz = __dmul_rn(sx, sz), syz = __dmul_rn(sy, sz);
+#define E_(ii, jj, kk) e[(size_t)(ii) + (size_t)cnx * ((size_t)(jj) + (size_t)cny * (size_t)(kk))]
+        return lerp(lerp(lerp(E_(I, J, K), __dmul_rn(sx, E_(Ip, J, K))),
+                         lerp(__dmul_rn(sy, E_(I, Jp, K)), __dmul_rn(sxy, E_(Ip, Jp, K)))),
+                    lerp(lerp(__dmul_rn(sz, E_(I, J, Kp)), __dmul_rn(sxz, E_(Ip, J, Kp))),
+                         lerp(__dmul_rn(syz, E_(I, Jp, Kp)), __dmul_rn(__dmul_rn(sxy, sz), E_(Ip, Jp, Kp)))));
+#undef E_
+    }
     const int Ip = far_index(I, i & 1, cnx, L.bcx);
     const int Jp = far_index(J, j & 1, cny, L.bcy);
     const int Kp = far_index(K, k & 1, cnz, L.bcz);

@@ -1,0 +1,148 @@
+"""GPU parity of per-side boundary conditions with Dirichlet walls (mg_create6; SURVEY 8(f) rank 3,
+DESIGN.md R24): the CUDA path (level-generic kernels with wall logic) against the CPU
+oracle (mgo_create6), element by element on identical seeded inputs.  Bars as in
+test_gpu_parity.py: single steps and cycles bit-exact, norms 1e-10, p after the solve 1e-9.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle.mgo import Oracle  # noqa: E402
+
+P, N, D = 0, 1, 2
+NORM_RTOL = 1e-10
+P_RTOL = 1e-9
+
+PAPER_BOX = (N, D, N, D, N, D)      # symmetry planes x-, y-; no-slip base z-; outflow x+, y+, z+
+
+CASES = [
+    ((32, 32, 32), PAPER_BOX),
+    ((48, 32, 24), (D, D, P, P, N, D)),
+    ((40, 24, 56), (P, P, D, N, D, D)),
+    ((64, 64, 64), (N, N, N, N, N, D)),
+    ((72, 40, 36), (D, N, N, N, P, P)),
+]
+
+
+@pytest.fixture(scope="module")
+def mgmod():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2605_30082_b200 as m
+    return m
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+
+
+def host(t):
+    return t.detach().cpu().numpy()
+
+
+def random_rho(uniform, seed, shape):
+    return np.exp(uniform(seed, shape, np.log(1.2), np.log(998.0)))
+
+
+def pair(mgmod, n, bc, nu=(2, 2), rho=None, coarse_sweeps=32, cycle_type=0):
+    o = Oracle(n, 1.0 / n[0], bc, nu[0], nu[1], coarse_sweeps)
+    g = mgmod.Multigrid(n, 1.0 / n[0], bc, nu[0], nu[1], coarse_sweeps)
+    o.set_cycle_type(cycle_type)
+    g.set_cycle_type(cycle_type)
+    if rho is not None:
+        o.set_density(rho)
+        g.set_density(dev(rho))
+    return o, g
+
+
+@pytest.mark.parametrize("n,bc", CASES)
+def test_steps_bit_exact_with_dirichlet_walls(mgmod, uniform, n, bc):
+    shp = (n[2], n[1], n[0])
+    o, g = pair(mgmod, n, bc, rho=random_rho(uniform, 121, shp))
+    assert o.num_levels == g.num_levels
+    for lvl in range(o.num_levels):
+        lshp = o.level_shape(lvl)
+        for bo, bg in zip(o.faces(lvl), g.level_faces(lvl)):        # minus faces incl. the minus walls
+            assert np.array_equal(bo, host(bg)), f"faces level {lvl}"
+        f, p0 = uniform(130 + lvl, lshp), uniform(140 + lvl, lshp)
+        po, pg, fd = p0.copy(), dev(p0), dev(f)
+        for colour in (0, 1, 0):
+            o.smooth_half(colour, f, po, lvl)
+            g.level_smooth_half(lvl, colour, fd, pg)
+            assert np.array_equal(po, host(pg)), f"half sweep colour {colour} level {lvl}"
+        # the residual sees every wall coefficient (plus walls included)
+        assert np.array_equal(o.residual_level(f, po, lvl), host(g.level_residual(lvl, fd, pg))), f"residual level {lvl}"
+        if lvl < o.num_levels - 1:
+            fc_o = o.restrict(o.residual_level(f, po, lvl), lvl)
+            assert np.array_equal(fc_o, host(g.level_residual_restrict(lvl, fd, pg)))
+            e = uniform(150 + lvl, o.level_shape(lvl + 1))
+            o.prolong_add(e, po, lvl)
+            g.level_prolong_add(lvl, dev(e), pg)
+            assert np.array_equal(po, host(pg)), f"prolong level {lvl}"
+
+
+@pytest.mark.parametrize("n,bc", CASES)
+@pytest.mark.parametrize("cycle_type", [0, 1], ids=["V", "F"])
+def test_cycles_bit_exact_with_dirichlet_walls(mgmod, uniform, n, bc, cycle_type):
+    shp = (n[2], n[1], n[0])
+    o, g = pair(mgmod, n, bc, nu=(3, 3), rho=random_rho(uniform, 122, shp), coarse_sweeps=8, cycle_type=cycle_type)
+    f = uniform(123, shp) + 0.25          # non-singular: the rhs need not be mean-free
+    po, pg, fd = np.zeros(shp), dev(np.zeros(shp)), dev(f)
+    for cyc in range(3):
+        o.vcycle(f, po)
+        g.vcycle(fd, pg)
+        assert np.array_equal(po, host(pg)), f"cycle {cyc}"
+    assert g.residual(fd, pg) == pytest.approx(o.residual(f, po), rel=NORM_RTOL)
+
+
+def test_solve_on_the_papers_box(mgmod, uniform):
+    """Drop-film densities in the paper's box: no-slip base, symmetry planes, outflow planes."""
+    from workloads import make_workload
+
+    w = make_workload(3, 64)
+    o, g = pair(mgmod, w.n, PAPER_BOX, nu=(w.nu1, w.nu2), rho=w.rho)
+    f = w.rhs + 0.1                        # no compatibility condition with a Dirichlet wall
+    po = np.zeros(o.shape)
+    so, co, ro, ho = o.solve(f, po, w.rtol, 60)
+    pg = dev(np.zeros(o.shape))
+    sg, cg, rg, hg = g.solve(dev(f), pg, w.rtol, 60)
+    assert so == 0 and (sg, cg) == (so, co)
+    hg = np.array(hg)
+    assert np.all(np.abs(hg / ho - 1) <= NORM_RTOL), (hg, ho)
+    pgh = host(pg)
+    assert np.abs(pgh - po).max() <= P_RTOL * np.abs(po).max()
+    assert abs(po.mean()) > 1e-6 * np.abs(po).max()          # no mean was removed on either side
+
+
+def test_dirichlet_solver_refuses_what_it_does_not_define(mgmod):
+    from paper_2605_30082_b200 import binding as B
+
+    g = mgmod.Multigrid((16, 16, 16), 1.0 / 16, PAPER_BOX)
+    for key in (B.MG_OPT_KERNELS, B.MG_OPT_COARSE_CTA):
+        with pytest.raises(B.MgError):
+            g.set_option(key, 1)
+    z = torch.zeros(g.shape, dtype=torch.float64, device="cuda:0")
+    with pytest.raises(B.MgError):
+        g.project_rhs(z, z, z, 1.0, z.clone())
+    for bad in [(P, N, P, P, P, P), (3, 3, N, N, N, N)]:
+        with pytest.raises(B.MgError):
+            mgmod.Multigrid((16, 16, 16), 1.0 / 16, bad)
+
+
+def test_six_entry_form_without_dirichlet_is_the_streaming_path(mgmod, uniform):
+    """(P,P,P,P,N,N) through mg_create6 = (P,P,N) through mg_create: same kernels, same bits."""
+    n = (64, 64, 64)
+    shp = (64, 64, 64)
+    rho = random_rho(uniform, 124, shp)
+    f = uniform(125, shp)
+    f -= f.mean()
+    outs = []
+    for bc in ((P, P, N), (P, P, P, P, N, N)):
+        g = mgmod.Multigrid(n, 1.0 / 64, bc, 3, 3)
+        g.set_density(dev(rho))
+        p = dev(np.zeros(shp))
+        g.vcycle(dev(f), p)
+        outs.append(host(p))
+    assert np.array_equal(outs[0], outs[1])
