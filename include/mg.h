@@ -155,6 +155,21 @@ int mg_residual(mg_handle *s, const double *rhs_dev, const double *p_dev,
 int mg_solve(mg_handle *s, const double *rhs_dev, double *p_dev, double rtol, int max_cycles,
              int *cycles_host, double *relres_host, double *hist_host);
 
+/* MG-preconditioned conjugate gradients (R22, C12-C14; the paper
+ * only names "the Multigrid").  Preconditioner z = M r = ONE symmetric cycle from
+ * z = 0: nu1 red->black sweeps, residual, restriction (1/8) P^T (the adjoint of the trilinear
+ * prolongation), coarse correction, prolongation, nu2 = nu1 black->red sweeps; on the coarsest
+ * level coarse_sweeps sweeps in each order.  mg_solve_pcg: r = f - A p, z = M r, d = z, then per
+ * iteration q = A d, alpha = r.z / d.q, p += alpha d, r -= alpha q, stop when ||r|| <= rtol ||r_0||
+ * (r of the recurrence), z = M r, beta = r.z' / r.z, d = z + beta d.  Arguments, return values and
+ * hist_host[0..iterations] as mg_solve; four more level-0 arrays are allocated on first use.
+ * MG_EINVAL if nu1 != nu2 or the solver has a Dirichlet side.  On the paper's workloads this
+ * iteration needs more work than mg_solve; it is here for completeness. */
+int mg_solve_pcg(mg_handle *s, const double *rhs_dev, double *p_dev, double rtol, int max_iter,
+                 int *iters_host, double *relres_host, double *hist_host);
+/* z_dev = M r_dev (one symmetric cycle from zero).  Asynchronous on the stream. */
+int mg_precondition(mg_handle *s, const double *r_dev, double *z_dev);
+
 /* End-to-end variant on HOST buffers (N doubles each; pinned memory makes the copies
  * asynchronous): copies rhs_host and, if non-NULL, rho_host to the device (then also
  * runs mg_set_density), solves from the initial guess p = 0, copies the zero-mean
@@ -215,6 +230,8 @@ int mg_level_smooth_restrict(mg_handle *s, int level, int sweeps, const double *
  * last post-sweep of mg_solve's cycle with step A7 fused behind it.  Synchronises the stream. */
 int mg_level_smooth_norm(mg_handle *s, int sweeps, const double *f_dev, double *p_dev, double *norm2_host);
 /* p += trilinear prolongation of e (e on level+1, p on level) */
+/* fc = (1/8) P^T r (C14), level -> level + 1 */
+int mg_level_restrict_adj(mg_handle *s, int level, const double *r_dev, double *fc_dev);
 int mg_level_prolong_add(mg_handle *s, int level, const double *e_dev, double *p_dev);
 
 #ifdef __cplusplus

@@ -37,6 +37,9 @@ SIGNATURES = {
     "mg_vcycle": (C.c_int, [_vp, _dp, _dp]),
     "mg_residual": (C.c_int, [_vp, _dp, _dp, _dp, _hp]),
     "mg_solve": (C.c_int, [_vp, _dp, _dp, C.c_double, C.c_int, _ip, _hp, _hp]),
+    "mg_solve_pcg": (C.c_int, [_vp, _dp, _dp, C.c_double, C.c_int, _ip, _hp, _hp]),
+    "mg_precondition": (C.c_int, [_vp, _dp, _dp]),
+    "mg_level_restrict_adj": (C.c_int, [_vp, C.c_int, _dp, _dp]),
     "mg_solve_host": (C.c_int, [_vp, _vp, _vp, _vp, C.c_double, C.c_int, _ip, _hp, _hp]),
     "mg_project_rhs": (C.c_int, [_vp, _dp, _dp, _dp, C.c_double, _dp]),
     "mg_project_correct": (C.c_int, [_vp, _dp, C.c_double, _dp, _dp, _dp]),
@@ -208,6 +211,27 @@ class Multigrid:
         if st < 0:
             raise MgError(st)
         return st, cyc.value, rel.value, list(hist[: cyc.value + 1])
+
+    def solve_pcg(self, rhs, p, rtol, max_iter):
+        """MG-preconditioned CG: returns (status, iterations, relres, hist[0..iterations])."""
+        it, rel = C.c_int(), C.c_double()
+        hist = (C.c_double * (max_iter + 1))()
+        st = lib().mg_solve_pcg(self._h, _ptr(rhs, self.shape), _ptr(p, self.shape), float(rtol),
+                                int(max_iter), C.byref(it), C.byref(rel), hist)
+        if st < 0:
+            raise MgError(st)
+        return st, it.value, rel.value, list(hist[: it.value + 1])
+
+    def precondition(self, r, z):
+        _chk(lib().mg_precondition(self._h, _ptr(r, self.shape), _ptr(z, self.shape)))
+        return z
+
+    def level_restrict_adj(self, level, r):
+        import torch
+
+        fc = torch.empty(self.level_shape(level + 1), dtype=torch.float64, device=self.device)
+        _chk(lib().mg_level_restrict_adj(self._h, level, _ptr(r, self.level_shape(level)), _ptr(fc)))
+        return fc
 
     def solve_host(self, rho_host, rhs_host, p_host, rtol, max_cycles):
         """Host-buffer variant: CPU torch tensors (ideally pinned) of shape (nz,ny,nx)."""
