@@ -312,6 +312,7 @@ def measure_rank(args, w, wname, rank, local, dist):
         # below is one or two launches of the named kernel, counted by the library)
         kern = {}
         p_d.zero_()
+        g.set_option(B.MG_OPT_SWEEP_FUSE, 3)
         t, nl = timed(lambda: g.level_smooth(0, 4, rhs_d, p_d), 10)
         kern["k_rbt<NS=2> two sweeps per pass"] = {"ms": t / nl, "bytes_per_cell": 32.0, "sweeps_per_launch": 2}
         g.set_option(B.MG_OPT_SWEEP_FUSE, 1)
@@ -446,16 +447,19 @@ def assemble_line(args, w, wname, world, m, t_ms, t_e2e_ms, cycles_all, e2e_cycl
     for name, k in m.get("kernels", {}).items():
         ach = k["bytes_per_cell"] * N / (k["ms"] * 1e-3) / 1e9
         kernels[name] = dict(k, achieved_gbs=ach, frac=ach / peak)
-    dom_name = "k_rbt<NS=2> two sweeps per pass"
+    # the cycle uses the two-sweep pass on level 0 from 2^26 cells (mg.cu use_fuse2), the one-sweep pass below
+    fused = N >= (1 << 26)
+    dom_name = "k_rbt<NS=2> two sweeps per pass" if fused else "k_rbt<NS=1> one sweep per pass"
     dom = kernels.get(dom_name)
     roof = {"bound": "hbm", "kernel": dom_name + " (level 0, p_in -> p_out: 32 B/cell per launch)",
             "achieved": dom["achieved_gbs"] if dom else None, "peak": peak, "unit": "GB/s",
             "frac": dom["frac"] if dom else None, "traffic": None, "peak_source": peak_src,
             "bytes_per_launch": 32.0 * N, "ms_per_launch": dom["ms"] if dom else None,
-            "note": "dominant by share of the V-cycle (2 launches); two red-black sweeps per HBM pass, so "
-                    "its bytes per second are lower than the one-sweep pass's although each sweep is faster: "
-                    "the fused pass is bound by shared-memory bandwidth and latency, not by HBM (DESIGN.md 4.1)",
-            "per_sweep_equivalent_frac": (2 * dom["frac"]) if dom else None,
+            "note": ("dominant by share of the V-cycle (2 launches); two red-black sweeps per HBM pass, so "
+                     "its bytes per second are lower than the one-sweep pass's although each sweep is faster: "
+                     "the fused pass is bound by shared-memory bandwidth and latency, not by HBM (DESIGN.md 4.1)")
+                    if fused else "dominant by share of the V-cycle; one red-black sweep per HBM pass at this size",
+            "per_sweep_equivalent_frac": ((2 if fused else 1) * dom["frac"]) if dom else None,
             "kernels": kernels}
     if list(w.n) == [512, 512, 512]:
         roof["traffic"] = NCU_TRAFFIC_512["bytes"]

@@ -63,11 +63,17 @@ enum {
                                1 = fused streaming kernels, TMA-staged sweeps (default)      */
     MG_OPT_GRAPH = 2,       /* 1 (default) = V-cycle replayed from a captured CUDA graph     */
     MG_OPT_COARSE_CTA = 3,  /* 1 (default) = levels <= 16^3 run in one persistent CTA       */
-    MG_OPT_SWEEP_FUSE = 4,  /* sweeps fused per pass of the TMA kernel: 1 or 2 (default) */
+    MG_OPT_SWEEP_FUSE = 4,  /* sweeps fused per pass of the TMA kernel: 1; 2 (default) = two where it
+                               pays (level 0 from 2^26 cells, streamed stored-face levels);
+                               3 = two wherever the kernel runs */
     MG_OPT_TAIL_FUSION = 5, /* 1 (default) = residual+restriction fused behind the last pre-sweep
                                and, in mg_solve, sum r^2 behind the last post-sweep, on level 0;
                                2 = the restriction tail on the streamed stored-face levels too;
                                0 = separate passes */
+    MG_OPT_PROLONG_FUSE = 7, /* 1 = prolongation + correction fused in front of the first post-sweep
+                               of level 0 (mg_vcycle; one pass of the TMA kernel whose p plane is
+                               staged as p + P e); 0 (default) = separate prolongation pass, which
+                               measured faster */
     MG_OPT_FACE_STREAM_LOG2 = 6 /* stored-face levels (>= 1) with at least 2^value cells use the
                                TMA kernel, smaller ones two half-sweep launches per sweep
                                (default 24; 0 = every level the kernel can tile) */
@@ -230,6 +236,10 @@ int mg_level_smooth_restrict(mg_handle *s, int level, int sweeps, const double *
  * last post-sweep of mg_solve's cycle with step A7 fused behind it.  Synchronises the stream. */
 int mg_level_smooth_norm(mg_handle *s, int sweeps, const double *f_dev, double *p_dev, double *norm2_host);
 /* p += trilinear prolongation of e (e on level+1, p on level) */
+/* p <- `sweeps` (>= 1) sweeps of (p + P e): prolongation, correction and the first sweep in one
+ * pass where the TMA kernel runs (level 0), otherwise mg_level_prolong_add + mg_level_smooth */
+int mg_level_prolong_smooth(mg_handle *s, int level, int sweeps, const double *e_dev, const double *f_dev,
+                            double *p_dev);
 /* fc = (1/8) P^T r (C14), level -> level + 1 */
 int mg_level_restrict_adj(mg_handle *s, int level, const double *r_dev, double *fc_dev);
 int mg_level_prolong_add(mg_handle *s, int level, const double *e_dev, double *p_dev);

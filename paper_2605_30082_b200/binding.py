@@ -15,6 +15,7 @@ MG_EINVAL, MG_ENOMEM, MG_ECUDA, MG_EINCOMPATIBLE, MG_EDIVERGED = -1, -2, -3, -4,
 MG_BC_PERIODIC, MG_BC_NEUMANN = 0, 1
 MG_OPT_KERNELS, MG_OPT_GRAPH, MG_OPT_COARSE_CTA, MG_OPT_SWEEP_FUSE, MG_OPT_TAIL_FUSION = 1, 2, 3, 4, 5
 MG_OPT_FACE_STREAM_LOG2 = 6
+MG_OPT_PROLONG_FUSE = 7
 MG_CYCLE_V, MG_CYCLE_F, MG_CYCLE_W = 0, 1, 2
 MG_STAT_KERNEL_LAUNCHES, MG_STAT_WORKSPACE_BYTES, MG_STAT_LAUNCHES_PER_VCYCLE = 1, 2, 3
 
@@ -39,6 +40,7 @@ SIGNATURES = {
     "mg_solve": (C.c_int, [_vp, _dp, _dp, C.c_double, C.c_int, _ip, _hp, _hp]),
     "mg_solve_pcg": (C.c_int, [_vp, _dp, _dp, C.c_double, C.c_int, _ip, _hp, _hp]),
     "mg_precondition": (C.c_int, [_vp, _dp, _dp]),
+    "mg_level_prolong_smooth": (C.c_int, [_vp, C.c_int, C.c_int, _dp, _dp, _dp]),
     "mg_level_restrict_adj": (C.c_int, [_vp, C.c_int, _dp, _dp]),
     "mg_solve_host": (C.c_int, [_vp, _vp, _vp, _vp, C.c_double, C.c_int, _ip, _hp, _hp]),
     "mg_project_rhs": (C.c_int, [_vp, _dp, _dp, _dp, C.c_double, _dp]),
@@ -312,6 +314,11 @@ class Multigrid:
         nrm = C.c_double()
         _chk(lib().mg_level_smooth_norm(self._h, sweeps, _ptr(f, self.shape), _ptr(p, self.shape), C.byref(nrm)))
         return nrm.value
+
+    def level_prolong_smooth(self, level, sweeps, e, f, p):
+        _chk(lib().mg_level_prolong_smooth(self._h, level, int(sweeps), _ptr(e, self.level_shape(level + 1)),
+                                           _ptr(f, self.level_shape(level)), _ptr(p, self.level_shape(level))))
+        return p
 
     def level_prolong_add(self, level, e, p):
         _chk(lib().mg_level_prolong_add(self._h, level, _ptr(e, self.level_shape(level + 1)),

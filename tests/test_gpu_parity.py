@@ -45,7 +45,7 @@ def pair(mgmod, n, h, bc, nu=(2, 2), rho=None, coarse_sweeps=32, **opts):
     from paper_2605_30082_b200 import binding as B
     for key, name in ((B.MG_OPT_KERNELS, "kernels"), (B.MG_OPT_GRAPH, "graph"), (B.MG_OPT_COARSE_CTA, "coarse_cta"),
                       (B.MG_OPT_TAIL_FUSION, "tails"), (B.MG_OPT_SWEEP_FUSE, "fuse"),
-                      (B.MG_OPT_FACE_STREAM_LOG2, "face_log2")):
+                      (B.MG_OPT_FACE_STREAM_LOG2, "face_log2"), (B.MG_OPT_PROLONG_FUSE, "head")):
         if name in opts:
             g.set_option(key, opts[name])
     if "cycle_type" in opts:
@@ -161,11 +161,30 @@ def test_fused_norm_tail(mgmod, uniform, n, bc, sweeps):
     assert nrm == pytest.approx(o.residual(f, po), rel=NORM_RTOL)
 
 
-@pytest.mark.parametrize("fuse", [1, 2])
+@pytest.mark.parametrize("n,bc", TAIL_SHAPES + [((128, 64, 48), (P, N, P))])
+@pytest.mark.parametrize("sweeps", [1, 2, 3])
+def test_fused_prolongation_head_bit_exact(mgmod, uniform, n, bc, sweeps):
+    """SURVEY 8(a) A5 + A6: prolongation, correction and the first post-sweep in one pass of the TMA
+    kernel (the p plane is staged as p_old + P e), then the remaining sweeps; p bit-exact.
+    (MG_OPT_PROLONG_FUSE = 1; off by default because the separate prolongation pass is faster.)"""
+    shp = (n[2], n[1], n[0])
+    o, g = pair(mgmod, n, 1.0 / n[0], bc, rho=random_rho(uniform, 54, shp), head=1)
+    f, p0 = uniform(55, shp), uniform(56, shp)
+    e = uniform(57, o.level_shape(1))
+    po = p0.copy()
+    o.prolong_add(e, po, 0)
+    for _ in range(sweeps):
+        o.sweep(f, po, 0)
+    pg = dev(p0)
+    g.level_prolong_smooth(0, sweeps, dev(e), dev(f), pg)
+    assert np.array_equal(po, host(pg))
+
+
+@pytest.mark.parametrize("fuse", [1, 2, 3])
 @pytest.mark.parametrize("sweeps", [2, 4, 5])
 def test_two_sweeps_fused_per_pass_bit_exact(mgmod, uniform, sweeps, fuse):
-    """MG_OPT_SWEEP_FUSE = 2 (default): temporal blocking, two red-black sweeps per pass of
-    k_rbt<2>; = 1: one sweep per pass."""
+    """MG_OPT_SWEEP_FUSE = 3: temporal blocking, two red-black sweeps per pass of k_rbt<2> at every
+    size; = 2 (default): where it pays (not at this size); = 1: one sweep per pass."""
     from paper_2605_30082_b200 import binding as B
     n, bc = (136, 72, 96), (P, N, P)
     shp = (n[2], n[1], n[0])
@@ -196,7 +215,7 @@ FACE_SHAPES = [
 
 
 @pytest.mark.parametrize("n,bc", FACE_SHAPES)
-@pytest.mark.parametrize("fuse", [1, 2])
+@pytest.mark.parametrize("fuse", [1, 3])
 def test_face_levels_streamed_bit_exact(mgmod, uniform, n, bc, fuse):
     shp = (n[2], n[1], n[0])
     o, g = pair(mgmod, n, 1.0 / n[0], bc, rho=random_rho(uniform, 61, shp), fuse=fuse, face_log2=0, tails=2)
@@ -241,12 +260,12 @@ def test_vcycle_face_levels_streamed_bit_exact(mgmod, uniform, n, bc, nu, tails)
 # V-cycles: every kernel-selection combination gives the oracle's iterate bit for bit
 # --------------------------------------------------------------------------- #
 OPTS = [dict(kernels=k, graph=gr, coarse_cta=c) for k, gr, c in itertools.product((0, 1), (0, 1), (0, 1))]
-OPTS += [dict(kernels=1, graph=1, coarse_cta=1, tails=0),
-         dict(kernels=1, graph=0, coarse_cta=1, fuse=1)]
+OPTS += [dict(kernels=1, graph=1, coarse_cta=1, tails=0), dict(kernels=1, graph=1, coarse_cta=1, head=1),
+         dict(kernels=1, graph=0, coarse_cta=1, fuse=1), dict(kernels=1, graph=1, coarse_cta=1, fuse=3)]
 
 
 @pytest.mark.parametrize("n,bc", SHAPES[:5] + SHAPES[7:])
-@pytest.mark.parametrize("opts", OPTS, ids=lambda d: "k%d-g%d-c%d-t%d-f%d" % (d["kernels"], d["graph"], d["coarse_cta"], d.get("tails", 1), d.get("fuse", 2)))
+@pytest.mark.parametrize("opts", OPTS, ids=lambda d: "k%d-g%d-c%d-t%d-f%d-h%d" % (d["kernels"], d["graph"], d["coarse_cta"], d.get("tails", 1), d.get("fuse", 2), d.get("head", 0)))
 @pytest.mark.parametrize("nu", [(2, 2), (3, 3), (1, 0)])
 def test_vcycle_bit_exact(mgmod, uniform, n, bc, opts, nu):
     h = 1.0 / n[0]
