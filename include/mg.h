@@ -8,7 +8,7 @@
  * mesh, with cell density from volume-fraction mixing (PAPER.md:47-52,
  * eq. 5) and "the Multigrid" as the solver.  The paper gives no
  * further detail; the operation is fixed by BASELINE.json `north_star` and the readings
- * R1-R19 / expression trees C1-C9 listed in DESIGN.md §3.
+ * R1-R24 / expression trees C1-C14 listed in DESIGN.md §3.
  * The call list is north_star's: mg_create(nx,ny,nz,h,bc), mg_set_density(rho),
  * mg_vcycle, mg_residual, mg_solve(rhs,p,rtol,max_cycles).
  *
@@ -16,8 +16,10 @@
  * x fastest, idx = i + nx*(j + ny*k), no ghost layers, no padding.
  *      (A p)_c = (1/h^2) * sum over the 6 faces of  beta_face * (p_nb - p_c)
  *      beta_face = 1/rho_face, rho_face = harmonic mean of the two cell densities
- * Per axis the boundary is periodic (wrap) or homogeneous Neumann (wall-face beta = 0).
- * A is singular (constants); rhs must be mean-free; mg_solve returns the zero-mean p.
+ * Per axis the boundary is periodic (wrap) or homogeneous Neumann (wall-face beta = 0);
+ * mg_create6 takes one type per side and adds Dirichlet walls (p = 0 on the wall face).
+ * Without a Dirichlet wall A is singular (constants): rhs must be mean-free and mg_solve
+ * returns the zero-mean p.
  * One V(nu1,nu2) cycle = nu1 red-black Gauss-Seidel sweeps (red = even i+j+k first),
  * residual, 8-child-mean restriction, recursion on the coarse grid from a zero guess,
  * cell-centred trilinear prolongation + correction, nu2 sweeps.  Coarse levels carry
@@ -90,7 +92,8 @@ enum {
 /* Bytes of device workspace a solver of this size needs (all levels, all scratch). */
 size_t mg_workspace_bytes(int nx, int ny, int nz);
 
-/* Create a solver.  bc[axis] in {MG_BC_PERIODIC, MG_BC_NEUMANN} for x,y,z (both sides
+/* north_star mg_create(nx,ny,nz,h,bc) (grid R2, R3, hierarchy R7, boundaries R5).
+ * Create a solver.  bc[axis] in {MG_BC_PERIODIC, MG_BC_NEUMANN} for x,y,z (both sides
  * of an axis share the type).  Builds the level list, allocates ALL storage once
  * (cf. the paper's memory-pool lesson) with cudaMalloc, sets rho == 1,
  * V(2,2), 32 coarsest sweeps, stream 0.
@@ -138,22 +141,30 @@ int mg_set_cycle_type(mg_handle *s, int type);
 int mg_set_option(mg_handle *s, int key, int value);
 int mg_get_stat(const mg_handle *s, int key, long long *value_host);
 
-/* Density field: rho_dev = N doubles, read-only, may be freed once the stream has
+/* Step A0 (north_star "face coefficients from harmonic-averaged cell density";
+ * density by volume-fraction mixing, eq. 5; readings R4, R8, C2, C3 of DESIGN.md).
+ * Density field: rho_dev = N doubles, read-only, may be freed once the stream has
  * passed this call.  The library derives and owns a = 0.5/rho (level 0) and the face
  * coefficients of every coarser level.  Synchronises the stream (validity check).
  * MG_EINVAL if any rho is <= 0 or non-finite (coefficients are then unspecified). */
 int mg_set_density(mg_handle *s, const double *rho_dev);
 
-/* One V(nu1,nu2) cycle in place on p_dev for right-hand side rhs_dev (N doubles each).
- * No mean removal, no norm.  Asynchronous on the stream. */
+/* Steps A1-A6, A8 (north_star "geometric multigrid V-cycle ... red-black Gauss-Seidel
+ * smoothing, residual, full-weighting restriction, trilinear prolongation and correction"; "the
+ * Multigrid"; readings R9-R14, R23, C4-C8).  One cycle of the set type (V by default)
+ * in place on p_dev for right-hand side rhs_dev (N doubles each), replayed from a CUDA graph.
+ * No mean removal, no norm.  Asynchronous on the stream.  MG_EINVAL for NULL or misaligned pointers. */
 int mg_vcycle(mg_handle *s, const double *rhs_dev, double *p_dev);
 
-/* r = rhs - A p.  Writes r to r_dev if non-NULL, and sqrt(sum r^2) to *norm2_host if
- * non-NULL (then the stream is synchronised). */
+/* Steps A2, A7 (north_star "residual", "residual-norm reductions"; R10, R15, C6, C9).
+ * r = rhs - A p.  Writes r to r_dev (N doubles, caller-owned) if non-NULL, and sqrt(sum r^2) to
+ * *norm2_host if non-NULL (then the stream is synchronised; the sum is a fixed two-stage tree,
+ * no atomics). */
 int mg_residual(mg_handle *s, const double *rhs_dev, const double *p_dev,
                 double *r_dev, double *norm2_host);
 
-/* V-cycles until ||rhs - A p||_2 <= rtol * ||rhs - A p_0||_2 or max_cycles.
+/* Step A7 + control (north_star mg_solve(rhs,p,rtol,max_cycles); R6, R15).
+ * Cycles until ||rhs - A p||_2 <= rtol * ||rhs - A p_0||_2 or max_cycles.
  * p_dev: in = initial guess, out = iterate with its arithmetic mean removed.
  * hist_host (NULL or >= max_cycles+1 doubles) receives ||r_k||_2, k = 0..cycles.
  * Returns MG_OK, MG_NOT_CONVERGED, MG_EINCOMPATIBLE (p untouched), MG_EDIVERGED.
