@@ -14,6 +14,7 @@
  *   beta_face = 1/rho_face with rho_face the harmonic mean of the two cell densities
  *             = (0.5/rho_a) + (0.5/rho_b)                                       [BJ; R4, C2]
  *   per axis: periodic (wrap) or homogeneous Neumann (wall-face beta = 0)       [R5]
+ *   per side (mgo_create6): also Dirichlet walls, p = 0 on the wall face        [R24]
  *   solved by geometric multigrid V(nu1,nu2) cycles: red-black Gauss-Seidel, residual,
  *   8-child-mean restriction, cell-centred trilinear prolongation + correction,
  *   coarse faces = mean of the 4 coincident fine faces, 4^3-ish coarsest level
@@ -22,7 +23,8 @@
  * It is an iteration, so the oracle follows the algorithm step by step in the order
  * and with the expression trees C1-C9 (no blocking, fusion or reordering).  Every level
  * stores explicit minus-face arrays bx,by,bz (bx[i,j,k] = face between (i-1,j,k) and
- * (i,j,k), wrap; a Neumann axis is a periodic axis whose wrap face is 0).
+ * (i,j,k); entry 0 of a non-periodic axis is the minus wall) and plus-wall arrays wx,wy,wz;
+ * the neighbour value beyond any wall is 0.0 (C2).
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): closed-form eigenvalues of sine/cosine
  * modes, symmetry / zero row+column sums, the layered-medium prefix-sum solution,
@@ -31,10 +33,17 @@
  * The coarse-face rule C3 is pinned value by value against numpy slices of the finer level's
  * faces on a fully 3-D random density (test_coarse_faces_brute_force_3d); the coarsest-level
  * sweep count against a one-level hierarchy (test_coarsest_level_runs_exactly_coarse_sweeps_sweeps).
+ * F- and W-cycles (R23): recursion over the pinned single steps bit for bit, visit counts, dense
+ * 16^3 solve (test_oracle_cycles.py).  Dirichlet walls (R24): closed-form eigenmodes of all side
+ * pairs, wall values and sides, coarse walls by brute force, layered medium with a Dirichlet top,
+ * dense non-singular solve, ghost weights, second-order convergence (test_oracle_bc6.py).
+ * MG-preconditioned CG (R22): adjoint identity, symmetry of M, dense solve (test_oracle_pcg.py).
+ * Projection steps (R21): linear fields, Gauss theorem, div(u_new)/dt = f - A p (test_oracle_projection.py).
  * PARITY UNPINNED (CHOICES among readings on which the paper is silent, not functions: what
  * the code computes under each choice is pinned): that R8 is the 4-face mean,
  * that R13's default is 32 sweeps, that R11 is the 8-child mean among the "full-weighting"
- * readings, R18 (sphere position in the input recipe).
+ * readings, R18 (sphere position in the input recipe), R21's staggering convention, R22's
+ * symmetric coarsest solve, R24's reading of "continuous" planes as p = 0 on the wall face.
  *
  * All pointers are HOST pointers to dense fp64 arrays, idx = i + nx*(j + ny*k).
  */
