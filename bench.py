@@ -473,6 +473,9 @@ def assemble_line(args, w, wname, world, m, t_ms, t_e2e_ms, cycles_all, e2e_cycl
                   "l2": f"inputs larger than L2 ({3 * N * 8 / 1e6:.0f} MB resident vs 126 MB)"},
         "time_to_rtol_ms": m["t_solve_ms"], "set_density_ms": m["t_setrho_ms"],
         "f_cycle": m.get("f_cycle"),
+        "time_to_rtol_best": (lambda fc: {"ms": min(m["t_solve_ms"], fc["time_to_rtol_ms"]),
+                                          "cycle": "F" if fc["time_to_rtol_ms"] < m["t_solve_ms"] else "V"})(m["f_cycle"])
+                             if m.get("f_cycle") else None,
         "vcycle": {"ms": t_vc_ms, "gcell_updates_per_s": N * upd / (t_vc_ms * 1e-3) / 1e9,
                    "launches": m["launches_per_vcycle"],
                    "frac_of_B_sched_roofline": (bs / (peak * 1e9)) / (t_vc_ms * 1e-3),

@@ -90,7 +90,7 @@ def test_run_cuda_control_flow_world2_with_stubbed_solver(tmp_path):
     assert out["value"] == pytest.approx(n_cells * upd * (10 + 11) / 0.150 / 1e9)      # max over ranks: 150 ms
     assert out["ms_per_step"] == pytest.approx(75.0)
     assert out["e2e"]["value"] == pytest.approx(n_cells * upd * 8 / 0.400 / 1e9)
-    assert "cpu_baseline" not in out
+    assert "cpu_baseline" not in out and out["time_to_rtol_best"] is None and out["time_to_rtol_ms"] == 20.0
 
 
 def test_gpus_flag_spawns_ranks_when_no_launcher_did():
