@@ -113,9 +113,11 @@ int mg_create_in(int nx, int ny, int nz, double h, const int bc[3],
  * 2 (a_c + a_c) whose neighbour value is 0; coarse walls are the mean of the four finer wall
  * faces; the prolongation ghost is -e_boundary).  With a Dirichlet wall the system is
  * non-singular: mg_solve checks no compatibility and removes no mean.  Such a solver runs the
- * level-generic kernels (MG_OPT_KERNELS = 0, MG_OPT_COARSE_CTA = 0; switching them on returns
- * MG_EINVAL), and mg_project* return MG_EINVAL (the staggered velocity layout has no plus-wall
- * face).  Without a Dirichlet side this is mg_create / mg_create_in.  Errors as mg_create. */
+ * TMA sweep kernel on level 0 (ghost beyond a Dirichlet wall: a = 3 a_c, p = 0, never updated) and
+ * the level-generic kernels for the transfers and the coarser levels (MG_OPT_COARSE_CTA = 1
+ * returns MG_EINVAL); mg_project*, mg_solve_pcg and mg_precondition return MG_EINVAL (the
+ * staggered velocity layout has no plus-wall face; the symmetric cycle is defined for periodic
+ * and Neumann sides).  Without a Dirichlet side this is mg_create / mg_create_in.  Errors as mg_create. */
 int mg_create6(int nx, int ny, int nz, double h, const int bc6[6], mg_handle **out);
 int mg_create6_in(int nx, int ny, int nz, double h, const int bc6[6],
                   void *workspace_dev, size_t workspace_bytes, mg_handle **out);

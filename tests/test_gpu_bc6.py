@@ -19,6 +19,8 @@ PAPER_BOX = (N, D, N, D, N, D)      # symmetry planes x-, y-; no-slip base z-; o
 
 CASES = [
     ((32, 32, 32), PAPER_BOX),
+    ((96, 64, 48), PAPER_BOX),               # several tiles and z-chunks of the TMA kernel
+    ((64, 72, 32), (D, N, D, D, D, N)),
     ((48, 32, 24), (D, D, P, P, N, D)),
     ((40, 24, 56), (P, P, D, N, D, D)),
     ((64, 64, 64), (N, N, N, N, N, D)),
@@ -46,9 +48,12 @@ def random_rho(uniform, seed, shape):
     return np.exp(uniform(seed, shape, np.log(1.2), np.log(998.0)))
 
 
-def pair(mgmod, n, bc, nu=(2, 2), rho=None, coarse_sweeps=32, cycle_type=0):
+def pair(mgmod, n, bc, nu=(2, 2), rho=None, coarse_sweeps=32, cycle_type=0, kernels=1):
+    from paper_2605_30082_b200 import binding as B
+
     o = Oracle(n, 1.0 / n[0], bc, nu[0], nu[1], coarse_sweeps)
     g = mgmod.Multigrid(n, 1.0 / n[0], bc, nu[0], nu[1], coarse_sweeps)
+    g.set_option(B.MG_OPT_KERNELS, kernels)      # 1 (default): TMA sweeps on level 0; 0: level-generic kernels only
     o.set_cycle_type(cycle_type)
     g.set_cycle_type(cycle_type)
     if rho is not None:
@@ -84,10 +89,35 @@ def test_steps_bit_exact_with_dirichlet_walls(mgmod, uniform, n, bc):
 
 
 @pytest.mark.parametrize("n,bc", CASES)
-@pytest.mark.parametrize("cycle_type", [0, 1], ids=["V", "F"])
-def test_cycles_bit_exact_with_dirichlet_walls(mgmod, uniform, n, bc, cycle_type):
+@pytest.mark.parametrize("sweeps", [1, 2, 3])
+def test_level0_sweeps_and_tails_with_dirichlet_walls(mgmod, uniform, n, bc, sweeps):
+    """The TMA kernel on level 0 (k_rbt WALLS): sweeps, fused pairs, restriction and norm tails."""
     shp = (n[2], n[1], n[0])
-    o, g = pair(mgmod, n, bc, nu=(3, 3), rho=random_rho(uniform, 122, shp), coarse_sweeps=8, cycle_type=cycle_type)
+    o, g = pair(mgmod, n, bc, rho=random_rho(uniform, 126, shp))
+    f, p0 = uniform(127, shp), uniform(128, shp)
+    po = p0.copy()
+    for _ in range(sweeps):
+        o.sweep(f, po, 0)
+    pg = dev(p0)
+    g.level_smooth(0, sweeps, dev(f), pg)
+    assert np.array_equal(po, host(pg))
+    pg = dev(p0)
+    fc_g = g.level_smooth_restrict(0, sweeps, dev(f), pg)
+    assert np.array_equal(po, host(pg))
+    assert np.array_equal(o.restrict(o.residual_level(f, po, 0), 0), host(fc_g))
+    pg = dev(p0)
+    nrm = g.level_smooth_norm(sweeps, dev(f), pg)
+    assert np.array_equal(po, host(pg))
+    assert nrm == pytest.approx(o.residual(f, po), rel=NORM_RTOL)
+
+
+@pytest.mark.parametrize("n,bc", CASES)
+@pytest.mark.parametrize("cycle_type", [0, 1], ids=["V", "F"])
+@pytest.mark.parametrize("kernels", [0, 1])
+def test_cycles_bit_exact_with_dirichlet_walls(mgmod, uniform, n, bc, cycle_type, kernels):
+    shp = (n[2], n[1], n[0])
+    o, g = pair(mgmod, n, bc, nu=(3, 3), rho=random_rho(uniform, 122, shp), coarse_sweeps=8, cycle_type=cycle_type,
+                kernels=kernels)
     f = uniform(123, shp) + 0.25          # non-singular: the rhs need not be mean-free
     po, pg, fd = np.zeros(shp), dev(np.zeros(shp)), dev(f)
     for cyc in range(3):
@@ -120,9 +150,8 @@ def test_dirichlet_solver_refuses_what_it_does_not_define(mgmod):
     from paper_2605_30082_b200 import binding as B
 
     g = mgmod.Multigrid((16, 16, 16), 1.0 / 16, PAPER_BOX)
-    for key in (B.MG_OPT_KERNELS, B.MG_OPT_COARSE_CTA):
-        with pytest.raises(B.MgError):
-            g.set_option(key, 1)
+    with pytest.raises(B.MgError):
+        g.set_option(B.MG_OPT_COARSE_CTA, 1)
     z = torch.zeros(g.shape, dtype=torch.float64, device="cuda:0")
     with pytest.raises(B.MgError):
         g.project_rhs(z, z, z, 1.0, z.clone())
