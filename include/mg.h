@@ -114,8 +114,8 @@ int mg_create_in(int nx, int ny, int nz, double h, const int bc[3],
  * faces; the prolongation ghost is -e_boundary).  With a Dirichlet wall the system is
  * non-singular: mg_solve checks no compatibility and removes no mean.  Such a solver runs the
  * TMA sweep kernel on level 0 (ghost beyond a Dirichlet wall: a = 3 a_c, p = 0, never updated) and
- * the level-generic kernels for the transfers and the coarser levels (MG_OPT_COARSE_CTA = 1
- * returns MG_EINVAL); mg_project*, mg_solve_pcg and mg_precondition return MG_EINVAL (the
+ * the level-generic kernels for the transfers and the coarser levels down to the persistent
+ * coarse CTA; mg_project*, mg_solve_pcg and mg_precondition return MG_EINVAL (the
  * staggered velocity layout has no plus-wall face; the symmetric cycle is defined for periodic
  * and Neumann sides).  Without a Dirichlet side this is mg_create / mg_create_in.  Errors as mg_create. */
 int mg_create6(int nx, int ny, int nz, double h, const int bc6[6], mg_handle **out);

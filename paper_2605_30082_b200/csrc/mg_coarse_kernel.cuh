@@ -17,6 +17,7 @@
 // coefficients only, so it is formed once per launch and reused by every sweep.
 #pragma once
 #include "mg_common.cuh"
+#include "mg_ref_kernels.cuh"     // far_index6: prolongation ghosts beyond walls (R24)
 
 namespace mg {
 
@@ -29,7 +30,12 @@ struct CoarseArgs {
     int n[kCoarseMaxLevels][3];
     double h2[kCoarseMaxLevels], ih2[kCoarseMaxLevels];
     const double *bx[kCoarseMaxLevels], *by[kCoarseMaxLevels], *bz[kCoarseMaxLevels];
-    int bc[3];
+    int bc[3];           // axis has walls (not periodic)
+    // R24 (mg_create6 with a Dirichlet side): wall logic as in the level-generic kernels.  The
+    // plus-wall planes stay in global memory (n^2 values per axis, read through L1).
+    int gen;
+    int bcm[3], bcp[3];
+    const double *wx[kCoarseMaxLevels], *wy[kCoarseMaxLevels], *wz[kCoarseMaxLevels];
     int nu1, nu2, coarse_sweeps;
     int cycle_type;      // 0 = V, 1 = F, 2 = W (R23)
     int warm;            // 0: initial guess 0; 1: a later visit, the guess is read from p
@@ -54,6 +60,8 @@ struct CLv {
     int nx, ny, nz;
     double h2, ih2;
     double *p, *f, *bx, *by, *bz, *id;
+    int gen, wallx, wally, wallz;          // R24: walls with their own coefficient
+    const double *wx, *wy, *wz;
 };
 
 __device__ __forceinline__ CLv coarse_level(const CoarseArgs &A, int q, double *sm)
@@ -65,6 +73,8 @@ __device__ __forceinline__ CLv coarse_level(const CoarseArgs &A, int q, double *
     L.h2 = A.h2[q]; L.ih2 = A.ih2[q];
     const size_t n = (size_t)L.nx * L.ny * L.nz;
     L.p = sm + off; L.f = L.p + n; L.bx = L.f + n; L.by = L.bx + n; L.bz = L.by + n; L.id = L.bz + n;
+    L.gen = A.gen; L.wallx = A.gen && A.bc[0]; L.wally = A.gen && A.bc[1]; L.wallz = A.gen && A.bc[2];
+    L.wx = A.wx[q]; L.wy = A.wy[q]; L.wz = A.wz[q];
     return L;
 }
 
@@ -76,6 +86,15 @@ __device__ __forceinline__ double coarse_S(const CLv &L, const double *p, int i,
     const int cxm = i == 0 ? c + (L.nx - 1) * sx : c - sx, cxp = i == L.nx - 1 ? c - (L.nx - 1) * sx : c + sx;
     const int cym = j == 0 ? c + (L.ny - 1) * sy : c - sy, cyp = j == L.ny - 1 ? c - (L.ny - 1) * sy : c + sy;
     const int czm = k == 0 ? c + (L.nz - 1) * sz : c - sz, czp = k == L.nz - 1 ? c - (L.nz - 1) * sz : c + sz;
+    if (L.gen) {        // R24: a plus wall has its own coefficient, the value beyond any wall is 0.0
+        const bool xm = L.wallx && i == 0, xp = L.wallx && i == L.nx - 1;
+        const bool ym = L.wally && j == 0, yp = L.wally && j == L.ny - 1;
+        const bool zm = L.wallz && k == 0, zp = L.wallz && k == L.nz - 1;
+        double b[6] = { L.bx[c], xp ? L.wx[j + L.ny * k] : L.bx[cxp], L.by[c], yp ? L.wy[i + L.nx * k] : L.by[cyp],
+                        L.bz[c], zp ? L.wz[i + L.nx * j] : L.bz[czp] };
+        return stencil_S(b, xm ? 0.0 : p[cxm], xp ? 0.0 : p[cxp], ym ? 0.0 : p[cym], yp ? 0.0 : p[cyp],
+                         zm ? 0.0 : p[czm], zp ? 0.0 : p[czp]);
+    }
     double b[6] = { L.bx[c], L.bx[cxp], L.by[c], L.by[cyp], L.bz[c], L.bz[czp] };
     return stencil_S(b, p[cxm], p[cxp], p[cym], p[cyp], p[czm], p[czp]);
 }
@@ -86,6 +105,12 @@ __device__ __forceinline__ double coarse_D(const CLv &L, int i, int j, int k, in
     const int cxp = i == L.nx - 1 ? c - (L.nx - 1) : c + 1;
     const int cyp = j == L.ny - 1 ? c - (L.ny - 1) * sy : c + sy;
     const int czp = k == L.nz - 1 ? c - (L.nz - 1) * sz : c + sz;
+    if (L.gen) {
+        double b[6] = { L.bx[c], (L.wallx && i == L.nx - 1) ? L.wx[j + L.ny * k] : L.bx[cxp],
+                        L.by[c], (L.wally && j == L.ny - 1) ? L.wy[i + L.nx * k] : L.by[cyp],
+                        L.bz[c], (L.wallz && k == L.nz - 1) ? L.wz[i + L.nx * j] : L.bz[czp] };
+        return stencil_D(b);
+    }
     double b[6] = { L.bx[c], L.bx[cxp], L.by[c], L.by[cyp], L.bz[c], L.bz[czp] };
     return stencil_D(b);
 }
@@ -150,15 +175,32 @@ __device__ __forceinline__ int coarse_far(int I, int side, int n, int neumann)
 }
 
 // A5: p += trilinear prolongation of the coarse correction (C8)
-__device__ __forceinline__ void coarse_prolong_add(const CLv &L, const CLv &C, const int bc[3], int tid,
+__device__ __forceinline__ void coarse_prolong_add(const CLv &L, const CLv &C, const CoarseArgs &A, int tid,
                                                    int nthr)
 {
+    const int *bc = A.bc;
     const int n = L.nx * L.ny * L.nz;
     const double *e = C.p;
     for (int c = tid; c < n; c += nthr) {
         const int i = c % L.nx, r = c / L.nx;
         const int j = r % L.ny, k = r / L.ny;
         const int I = i >> 1, J = j >> 1, K = k >> 1;
+        if (A.gen) {        // R24: the value beyond a Dirichlet wall is -e_boundary (signs multiply over the axes)
+            double sx, sy, sz;
+            const int Ip = far_index6(I, i & 1, C.nx, A.bcm[0], A.bcp[0], sx);
+            const int Jp = far_index6(J, j & 1, C.ny, A.bcm[1], A.bcp[1], sy);
+            const int Kp = far_index6(K, k & 1, C.nz, A.bcm[2], A.bcp[2], sz);
+            const double sxy = __dmul_rn(sx, sy), sxz = __dmul_rn(sx, sz), syz = __dmul_rn(sy, sz);
+#define CE_(ii, jj, kk) e[(ii) + C.nx * ((jj) + C.ny * (kk))]
+            const double v =
+                lerp(lerp(lerp(CE_(I, J, K), __dmul_rn(sx, CE_(Ip, J, K))),
+                          lerp(__dmul_rn(sy, CE_(I, Jp, K)), __dmul_rn(sxy, CE_(Ip, Jp, K)))),
+                     lerp(lerp(__dmul_rn(sz, CE_(I, J, Kp)), __dmul_rn(sxz, CE_(Ip, J, Kp))),
+                          lerp(__dmul_rn(syz, CE_(I, Jp, Kp)), __dmul_rn(__dmul_rn(sxy, sz), CE_(Ip, Jp, Kp)))));
+#undef CE_
+            L.p[c] = __dadd_rn(L.p[c], v);
+            continue;
+        }
         const int Ip = coarse_far(I, i & 1, C.nx, bc[0]);
         const int Jp = coarse_far(J, j & 1, C.ny, bc[1]);
         const int Kp = coarse_far(K, k & 1, C.nz, bc[2]);
@@ -204,7 +246,7 @@ __device__ __forceinline__ void coarse_cycle(const CoarseArgs &A, double *sm, in
                 continue;
             }
         }
-        coarse_prolong_add(L, C, A.bc, tid, nthr);
+        coarse_prolong_add(L, C, A, tid, nthr);
         __syncthreads();
         coarse_sweeps(L, A.nu2, tid, nthr);
         --sp;
@@ -257,7 +299,7 @@ __global__ void __launch_bounds__(kCoarseThreads, 1) k_coarse_cta(CoarseArgs A)
     for (int q = A.nlev - 2; q >= 0; --q) {
         const CLv L = coarse_level(A, q, coarse_sm);
         const CLv C = coarse_level(A, q + 1, coarse_sm);
-        coarse_prolong_add(L, C, A.bc, tid, nthr);
+        coarse_prolong_add(L, C, A, tid, nthr);
         __syncthreads();
         coarse_sweeps(L, A.nu2, tid, nthr);
     }
