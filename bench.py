@@ -429,7 +429,7 @@ def measure_rank(args, w, wname, rank, local, dist):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel at 512^3, from the
 # `ncu --set full` capture summarised in the named file (bench.py itself never runs under ncu)
-NCU_TRAFFIC_512 = {"bytes": 4.272e9 + 1.114e9, "source": "profiles/r2b_cycle.md (k_rbt<NS=2>, 512^3)"}
+NCU_TRAFFIC_512 = {"bytes": 4.279e9 + 1.145e9, "source": "profiles/r2b_cycle.md (k_rbt<2,NONE,CELL>, 512^3: dram read + write)"}
 
 
 def assemble_line(args, w, wname, world, m, t_ms, t_e2e_ms, cycles_all, e2e_cycles_all):
