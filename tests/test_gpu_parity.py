@@ -161,6 +161,49 @@ def test_fused_norm_tail(mgmod, uniform, n, bc, sweeps):
     assert nrm == pytest.approx(o.residual(f, po), rel=NORM_RTOL)
 
 
+def _seeded_shapes(count, seed):
+    """Extents 4k in [32, 108] (x, y) and [16, 68] (z), so that there are at least two levels, with a
+    random boundary set: tile edges, shifted last tiles, patched images and z-chunk seams fall at
+    many different offsets."""
+    rng = np.random.default_rng(seed)
+    out = []
+    for _ in range(count):
+        n = (int(rng.integers(8, 28)) * 4, int(rng.integers(8, 28)) * 4, int(rng.integers(4, 18)) * 4)
+        out.append((n, tuple(int(b) for b in rng.integers(0, 2, size=3))))
+    return out
+
+
+@pytest.mark.parametrize("n,bc", _seeded_shapes(12, 20262))
+def test_tma_kernel_on_seeded_ragged_shapes(mgmod, uniform, n, bc):
+    """Every instance of the level-0 TMA kernel (one sweep, two sweeps per pass, restriction tail,
+    norm tail, prolongation head) on shapes drawn at random: p and the coarse rhs bit-exact."""
+    shp = (n[2], n[1], n[0])
+    o, g = pair(mgmod, n, 1.0 / n[0], bc, rho=random_rho(uniform, 301, shp), fuse=3, head=1)
+    f, p0 = uniform(302, shp), uniform(303, shp)
+    po = p0.copy()
+    for _ in range(3):
+        o.sweep(f, po, 0)
+    pg = dev(p0)
+    g.level_smooth(0, 3, dev(f), pg)                       # in-place sweep + one two-sweep pass
+    assert np.array_equal(po, host(pg))
+    pg = dev(p0)
+    fc_g = g.level_smooth_restrict(0, 3, dev(f), pg)       # two-sweep pass + one sweep with the tail
+    assert np.array_equal(po, host(pg))
+    assert np.array_equal(o.restrict(o.residual_level(f, po, 0), 0), host(fc_g))
+    pg = dev(p0)
+    nrm = g.level_smooth_norm(3, dev(f), pg)
+    assert np.array_equal(po, host(pg))
+    assert nrm == pytest.approx(o.residual(f, po), rel=NORM_RTOL)
+    e = uniform(304, o.level_shape(1))
+    po2 = p0.copy()
+    o.prolong_add(e, po2, 0)
+    for _ in range(2):
+        o.sweep(f, po2, 0)
+    pg = dev(p0)
+    g.level_prolong_smooth(0, 2, dev(e), dev(f), pg)
+    assert np.array_equal(po2, host(pg))
+
+
 @pytest.mark.parametrize("n,bc", TAIL_SHAPES + [((128, 64, 48), (P, N, P))])
 @pytest.mark.parametrize("sweeps", [1, 2, 3])
 def test_fused_prolongation_head_bit_exact(mgmod, uniform, n, bc, sweeps):
