@@ -227,11 +227,19 @@ __global__ void __launch_bounds__(RS_THREADS) k_resid_stream(RsArgs A)
 struct PrArgs {
     int nx, ny, nz;            // fine dims
     int cnx, cny, cnz;         // coarse dims
-    int bcx, bcy, bcz;
+    int bcx, bcy, bcz;         // axis has walls (clamped neighbour index)
+    int gen;                   // R24: some side is a Dirichlet wall (bcm / bcp = type per side)
+    int bcm[3], bcp[3];
     const double *e;
     const double *pin;
     double *pout;
 };
+
+// R24: a coarse value taken beyond a Dirichlet wall enters with sign -1 (ghost = -e_boundary)
+__device__ __forceinline__ double pr_sign(int I, int d, int n, int bc_minus, int bc_plus)
+{
+    return ((I + d < 0 && bc_minus == 2) || (I + d >= n && bc_plus == 2)) ? -1.0 : 1.0;
+}
 
 __device__ __forceinline__ int pr_nb(int I, int d, int n, int neumann)
 {
@@ -254,6 +262,15 @@ __global__ void __launch_bounds__(128) k_prolong_stream(PrArgs A)
         yj[d] = pr_nb(J, d - 1, A.cny, A.bcy);
         zk[d] = pr_nb(K, d - 1, A.cnz, A.bcz);
     }
+    double sx[3] = { 1.0, 1.0, 1.0 }, sy[3] = { 1.0, 1.0, 1.0 }, sz[3] = { 1.0, 1.0, 1.0 };
+    if (A.gen) {
+#pragma unroll
+        for (int d = 0; d < 3; d += 2) {
+            sx[d] = pr_sign(I, d - 1, A.cnx, A.bcm[0], A.bcp[0]);
+            sy[d] = pr_sign(J, d - 1, A.cny, A.bcm[1], A.bcp[1]);
+            sz[d] = pr_sign(K, d - 1, A.cnz, A.bcm[2], A.bcp[2]);
+        }
+    }
     // x-stage: X[s][dj][dk] = lerp_x(e[I], e[I -/+ 1]) on the 3x3 (J,K) neighbourhood
     double X[2][3][3];
 #pragma unroll
@@ -261,7 +278,13 @@ __global__ void __launch_bounds__(128) k_prolong_stream(PrArgs A)
 #pragma unroll
         for (int dj = 0; dj < 3; ++dj) {
             const double *row = A.e + (size_t)A.cnx * ((size_t)yj[dj] + (size_t)A.cny * (size_t)zk[dk]);
-            const double em = __ldg(row + xi[0]), ec = __ldg(row + xi[1]), ep = __ldg(row + xi[2]);
+            double em = __ldg(row + xi[0]), ec = __ldg(row + xi[1]), ep = __ldg(row + xi[2]);
+            if (A.gen) {        // each value carries the product of the signs of the axes on which it is far
+                const double syz = __dmul_rn(sy[dj], sz[dk]);
+                em = __dmul_rn(__dmul_rn(sx[0], syz), em);
+                ec = __dmul_rn(syz, ec);
+                ep = __dmul_rn(__dmul_rn(sx[2], syz), ep);
+            }
             X[0][dj][dk] = lerp(ec, em);
             X[1][dj][dk] = lerp(ec, ep);
         }
