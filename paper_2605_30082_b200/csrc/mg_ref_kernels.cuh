@@ -189,24 +189,6 @@ __global__ void k_residual_restrict(Lv L, const double *__restrict__ f,
                          __dadd_rn(__dadd_rn(r[4], r[5]), __dadd_rn(r[6], r[7]))));
 }
 
-// plain restriction of a given field (mg_level_* diagnostics only)
-__global__ void k_restrict(int cnx, int cny, int fnx, int fny, const double *__restrict__ r,
-                           double *__restrict__ fc)
-{
-    const int I = blockIdx.x * blockDim.x + threadIdx.x;
-    const int J = blockIdx.y * blockDim.y + threadIdx.y;
-    const int K = blockIdx.z;
-    if (I >= cnx || J >= cny) return;
-    double v[8];
-#pragma unroll
-    for (int q = 0; q < 8; ++q)
-        v[q] = r[(size_t)(2 * I + (q & 1)) +
-                 (size_t)fnx * ((size_t)(2 * J + ((q >> 1) & 1)) + (size_t)fny * (size_t)(2 * K + (q >> 2)))];
-    fc[(size_t)I + (size_t)cnx * ((size_t)J + (size_t)cny * (size_t)K)] = __dmul_rn(
-        0.125, __dadd_rn(__dadd_rn(__dadd_rn(v[0], v[1]), __dadd_rn(v[2], v[3])),
-                         __dadd_rn(__dadd_rn(v[4], v[5]), __dadd_rn(v[6], v[7]))));
-}
-
 // ---- A5: p += trilinear prolongation of e (C8) -----------------------------------
 __device__ __forceinline__ int far_index(int I, int side, int n, int neumann)
 {
