@@ -39,6 +39,9 @@
  * dense non-singular solve, ghost weights, second-order convergence (test_oracle_bc6.py).
  * MG-preconditioned CG (R22): adjoint identity, symmetry of M, dense solve (test_oracle_pcg.py).
  * Projection steps (R21): linear fields, Gauss theorem, div(u_new)/dt = f - A p (test_oracle_projection.py).
+ * mgo_solve's control (R15): r_0 and hist[0] from the incoming p != 0, every hist[k] replayed through
+ * apply, stop at the first k below rtol r_0, statuses for max_cycles = 0 and r_0 = 0
+ * (test_solve_measures_r0_from_the_incoming_p).
  * PARITY UNPINNED (CHOICES among readings on which the paper is silent, not functions: what
  * the code computes under each choice is pinned): that R8 is the 4-face mean,
  * that R13's default is 32 sweeps, that R11 is the 8-child mean among the "full-weighting"

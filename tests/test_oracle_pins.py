@@ -434,7 +434,49 @@ def test_config1_converges_to_known_solution():
     assert np.all(np.diff(hist) < 0)
     assert np.abs(p - w.p_exact).max() <= 1e-10
     # hist[k] really is ||f - A p_k||: recompute the last one independently via apply
-    assert hist[-1] == pytest.approx(np.linalg.norm((w.rhs - o.apply(p)).ravel()), rel=1e-6)
+    assert hist[-1] == pytest.approx(np.linalg.norm((w.rhs - o.apply(p)).ravel()), rel=1e-12)
+
+
+def test_solve_measures_r0_from_the_incoming_p(uniform):
+    """Pins R15 in mgo_solve: r_0 = ||f - A p_0|| of the INCOMING p (not ||f||), hist[0] is that
+    number, the stop is the first k with hist[k] <= rtol * hist[0], and the statuses of the two
+    degenerate calls.  Built from the pinned apply() and numpy's norm only.  p_0 is chosen so that
+    ||f - A p_0|| is about 1000 ||f||: with r_0 read as ||f|| the same rtol would need several
+    more cycles, with hist[0] = 2 r_0 one fewer could pass, so each misreading moves `cyc`."""
+    o = Oracle((16, 16, 16), 1.0 / 16, (P, N, P), 2, 2)
+    o.set_density(np.exp(uniform(301, o.shape, np.log(1.2), np.log(998.0))))
+    f = uniform(302, o.shape)
+    f -= f.mean()
+    p0 = 1000.0 * uniform(303, o.shape) * np.linalg.norm(f.ravel()) / np.linalg.norm(o.apply(uniform(303, o.shape)).ravel())
+    r0 = np.linalg.norm((f - o.apply(p0)).ravel())
+    assert r0 > 500.0 * np.linalg.norm(f.ravel())
+    rtol = 1e-4
+    p = p0.copy()
+    st, cyc, rel, hist = o.solve(f, p, rtol, 40)
+    assert st == mgo.OK and len(hist) == cyc + 1
+    assert hist[0] == pytest.approx(r0, rel=1e-13)
+    # every entry is the residual of the iterate it belongs to: replay the cycles by hand
+    q = p0.copy()
+    for k in range(1, cyc + 1):
+        o.vcycle(f, q)
+        assert hist[k] == pytest.approx(np.linalg.norm((f - o.apply(q)).ravel()), rel=1e-12)
+    # stop at the FIRST k below rtol * r0, measured against r0 of the incoming p
+    below = [k for k in range(cyc + 1) if hist[k] <= rtol * r0]
+    assert below == [cyc]
+    assert hist[cyc] > rtol * np.linalg.norm(f.ravel())          # ||f|| as r_0 would have gone on
+    assert hist[cyc - 1] > rtol * 2.0 * r0                        # 2 r_0 would still stop here or earlier ...
+    assert rel == pytest.approx(hist[cyc] / r0, rel=1e-13)        # ... but relres pins the denominator
+    assert np.array_equal(p, q - q.mean()) or np.abs(p - (q - q.mean())).max() <= 1e-13 * np.abs(q).max()
+    # max_cycles = 0: not converged, no cycle run, only the mean removed
+    p = p0.copy()
+    st, cyc0, rel0, hist0 = o.solve(f, p, rtol, 0)
+    assert st == mgo.NOT_CONVERGED and cyc0 == 0 and len(hist0) == 1
+    assert hist0[0] == pytest.approx(r0, rel=1e-13) and rel0 == 1.0
+    assert np.abs(p - (p0 - p0.mean())).max() <= 1e-13 * np.abs(p0).max()
+    # rhs = 0 from p = 0: r_0 = 0 counts as converged at once
+    z = np.zeros(o.shape)
+    st, cycz, relz, histz = o.solve(z, z.copy(), rtol, 5)
+    assert st == mgo.OK and cycz == 0 and list(histz) == [0.0] and relz == 0.0
 
 
 def test_level_counts_of_the_configs():
