@@ -220,6 +220,44 @@ int mg_project_correct(mg_handle *s, const double *p_dev, double dt, double *u_d
 int mg_project(mg_handle *s, double *u_dev, double *v_dev, double *w_dev, double dt, double *p_dev,
                double *rhs_dev, double rtol, int max_cycles, int *cycles_host, double *relres_host);
 
+/* ---- residual norm for callers that must not allocate (steps A2 + A7 on level 0; R10, R15, C2, C4, C6, C9).
+ * Some hosts of this library cannot call cudaMalloc at the point where they want a residual
+ * norm: a flow solver that, like the paper's (section 4.2), gave all device memory to
+ * its own pool at start-up has nothing left to allocate from, and a convergence monitor hooked
+ * into a running time loop must avoid the device-wide synchronisation cudaMalloc and cudaFree
+ * imply.  Every other call here needs a handle, and creating one allocates (mg_create the whole
+ * hierarchy; mg_create_in still pinned host memory).  This one call takes no handle and calls no
+ * cudaMalloc, cudaFree, cudaMallocHost or any other allocating routine; it only launches two
+ * kernels on `cuda_stream` (a cudaStream_t, NULL = default stream) and returns without waiting.
+ *
+ *   *norm2_dev = sqrt( sum over all cells of (rhs - A p)^2 ),  A built from rho as mg_set_density
+ *   does (a = 0.5/rho, face = a_c + a_nb, Neumann wall face = 0) with cell size h.
+ *
+ * Inputs rho_dev, rhs_dev, p_dev: nx*ny*nz doubles each on the CURRENT device, read-only, layout
+ * as everywhere in this header; rho must be finite and > 0 (not checked here).  Output norm2_dev:
+ * one double on the same device, written by the second kernel.  bc[axis] is MG_BC_PERIODIC or
+ * MG_BC_NEUMANN.  The value differs from mg_residual's norm only in how the partial sums are
+ * grouped (tests/test_zz_no_alloc.py holds the two to relative 1e-10).
+ *
+ * Scratch.  The per-block partial sums live in a fixed array compiled into the library (128 KB;
+ * every GPU that loads libmg holds it until the process ends), sized for at most
+ * MG_STATIC_MAX_CELLS = 2^27 cells (512^3, the paper's load per device).  A larger grid is
+ * refused with MG_EINVAL and mg_last_cuda_error() then says so; use mg_residual on a handle
+ * there.  All calls on one GPU share that array: calls whose kernels can overlap on the GPU
+ * (different streams without an ordering between them, several host threads) race on it and
+ * return garbage, so keep them on one stream or order them with events.  The array keeps the
+ * partial sums of the previous call; each call first overwrites every slot it later reads, so
+ * nothing has to be cleared and no call sees another's leftovers.
+ *
+ * First call on each device.  It looks up the device address of that array
+ * (cudaGetSymbolAddress, with this device current) and remembers it; later calls skip this.
+ * Make this first call during start-up, before any stream capture begins.
+ * Errors: MG_EINVAL (bad sizes as mg_create, bad bc, NULL pointer, too many cells), MG_ECUDA. */
+#define MG_STATIC_MAX_CELLS 134217728LL
+int mg_residual_norm_static(int nx, int ny, int nz, double h, const int bc[3],
+                            const double *rho_dev, const double *rhs_dev, const double *p_dev,
+                            double *norm2_dev, void *cuda_stream);
+
 const char *mg_strerror(int status);
 /* Text of the last CUDA error seen by this thread inside the library ("" if none). */
 const char *mg_last_cuda_error(void);

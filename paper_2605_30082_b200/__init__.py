@@ -11,5 +11,6 @@ from .binding import (  # noqa: F401
     MgError,
     Multigrid,
     lib,
+    residual_norm_static,
     workspace_bytes,
 )

@@ -46,6 +46,7 @@ SIGNATURES = {
     "mg_project_rhs": (C.c_int, [_vp, _dp, _dp, _dp, C.c_double, _dp]),
     "mg_project_correct": (C.c_int, [_vp, _dp, C.c_double, _dp, _dp, _dp]),
     "mg_project": (C.c_int, [_vp, _dp, _dp, _dp, C.c_double, _dp, _dp, C.c_double, C.c_int, _ip, _hp]),
+    "mg_residual_norm_static": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_double, _ip, _dp, _dp, _dp, _dp, _vp]),
     "mg_strerror": (C.c_char_p, [C.c_int]),
     "mg_last_cuda_error": (C.c_char_p, []),
     "mg_num_levels": (C.c_int, [_vp]),
@@ -78,10 +79,12 @@ def lib():
 
 
 class MgError(RuntimeError):
-    def __init__(self, code):
+    def __init__(self, code, detail=None):
         msg = lib().mg_strerror(code).decode()
         if code == MG_ECUDA:
             msg += ": " + lib().mg_last_cuda_error().decode()
+        elif detail:
+            msg += ": " + detail
         super().__init__(f"libmg error {code}: {msg}")
         self.code = code
 
@@ -107,6 +110,34 @@ def _ptr(t, shape=None):
         assert tuple(t.shape) == tuple(shape), (tuple(t.shape), tuple(shape))
     assert t.data_ptr() % 16 == 0, "device arrays must be 16-byte aligned (include/mg.h)"
     return t.data_ptr()
+
+
+MG_STATIC_MAX_CELLS = 1 << 27
+
+
+def residual_norm_static(n, h, bc, rho, rhs, p, out, stream=None):
+    """``out[0] = ||rhs - A p||_2`` through mg_residual_norm_static: no handle, and the library
+    allocates nothing (its scratch is a fixed array inside libmg, good for up to
+    MG_STATIC_MAX_CELLS cells; larger grids raise MgError(MG_EINVAL)).  Meant for callers that
+    cannot allocate device memory where they need the norm: a solver whose memory all sits in
+    its own pool, or a monitor inside a running time loop that must not trigger cudaMalloc's
+    device-wide synchronisation.  ``out`` is the caller's own 1-element CUDA float64 tensor;
+    the call is asynchronous on ``stream`` (default: torch's current stream).  Calls share the
+    scratch array, so do not let two of them overlap on one GPU."""
+    import torch
+
+    nx, ny, nz = (n, n, n) if isinstance(n, int) else n
+    shape = (int(nz), int(ny), int(nx))
+    assert isinstance(out, torch.Tensor) and out.is_cuda and out.dtype == torch.float64 and out.numel() == 1
+    bca = (C.c_int * 3)(*[int(b) for b in bc])
+    with torch.cuda.device(out.device):
+        st = stream if stream is not None else torch.cuda.current_stream(out.device)
+        code = lib().mg_residual_norm_static(int(nx), int(ny), int(nz), float(h), bca, _ptr(rho, shape),
+                                             _ptr(rhs, shape), _ptr(p, shape), out.data_ptr(), st.cuda_stream)
+    if code == MG_EINVAL and lib().mg_last_cuda_error():
+        raise MgError(code, lib().mg_last_cuda_error().decode())
+    _chk(code)
+    return out
 
 
 class Multigrid:
