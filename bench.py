@@ -291,15 +291,20 @@ def measure_rank(args, w, wname, rank, local, dist):
             p_d.zero_()
             return g.solve(rhs_d, p_d, w.rtol, max_cycles)
 
+        def median_solve(reps=5):
+            ts = sorted(timed(solve_once, 1, warm=0)[0] for _ in range(reps))
+            return ts[len(ts) // 2], ts
+
         g.set_density(rho_d)
-        m["t_solve_ms"], _ = timed(solve_once, 1, warm=0)
+        m["t_solve_ms"], m["t_solve_samples"] = median_solve()
         g.set_cycle_type(B.MG_CYCLE_F)
         solve_once()
-        t_f, _ = timed(solve_once, 1, warm=0)
+        t_f, t_f_all = median_solve()
         rf = solve_once()
         p_d.zero_()
         t_fc, _ = timed(lambda: g.vcycle(rhs_d, p_d), 10, warm=3)
         m["f_cycle"] = {"time_to_rtol_ms": t_f, "cycles": rf[1], "relres": rf[2], "ms_per_cycle": t_fc,
+                        "time_to_rtol_samples_ms": t_f_all,
                         "what": "the same solve with mg_set_cycle_type(MG_CYCLE_F): F(nu1,nu2) cycles"}
         g.set_cycle_type(B.MG_CYCLE_V)
 
@@ -323,8 +328,37 @@ def measure_rank(args, w, wname, rank, local, dist):
         t, nl = timed(lambda: g.level_prolong_add(0, e1_d, p_d), 10)
         kern["k_prolong_stream"] = {"ms": t / nl, "bytes_per_cell": 17.0}
         t, nl = timed(lambda: g.residual(rhs_d, p_d), 10)
-        kern["k_resid_stream<NORM> (+ k_final_sum)"] = {"ms": t, "bytes_per_cell": 24.0}
+        kern["mg_residual call: k_resid_stream<NORM> + k_final_sum + host fetch"] = {"ms": t, "bytes_per_cell": 24.0}
+        # the same streaming kernel alone (restriction variant: one launch, no host fetch)
+        t, nl = timed(lambda: g.level_residual_restrict(0, rhs_d, p_d), 10)
+        kern["k_resid_stream<RESTRICT>"] = {"ms": t / nl, "bytes_per_cell": 25.0}
+        # two sweeps with the restriction tail = k_rbt<1> (p -> q) + k_rbt<1,RESTRICT> (q -> p): no copy back;
+        # the tail pass is the call minus the one-sweep pass timed above
+        g.set_option(B.MG_OPT_SWEEP_FUSE, 1)
+        t, nl = timed(lambda: g.level_smooth_restrict(0, 2, rhs_d, p_d), 10)
+        g.set_option(B.MG_OPT_SWEEP_FUSE, 2)
+        if nl == 2:
+            kern["k_rbt<NS=1,RESTRICT> sweep + residual + restriction"] = {
+                "ms": t - kern["k_rbt<NS=1> one sweep per pass"]["ms"], "bytes_per_cell": 33.0, "sweeps_per_launch": 1,
+                "how": "2-launch call minus the one-sweep pass"}
         del e1_d
+        # level 1 (stored faces: p, bx, by, bz, f in, p out = 48 B per level-1 cell and pass)
+        if g.num_levels > 2 and g.level_shape(1)[0] * g.level_shape(1)[1] * g.level_shape(1)[2] >= (1 << 24):
+            n1 = g.level_shape(1)[0] * g.level_shape(1)[1] * g.level_shape(1)[2]
+            f1 = torch.randn(g.level_shape(1), dtype=torch.float64, device=devname)
+            p1 = torch.zeros(g.level_shape(1), dtype=torch.float64, device=devname)
+            e2_d = torch.zeros(g.level_shape(2), dtype=torch.float64, device=devname)
+            t, nl = timed(lambda: g.level_smooth(1, 4, f1, p1), 10)
+            kern["level 1: k_rbt<NS=2,FACES> two sweeps per pass"] = {"ms": t / nl, "bytes_per_cell": 48.0, "cells": n1, "sweeps_per_launch": 2}
+            g.set_option(B.MG_OPT_SWEEP_FUSE, 1)
+            t, nl = timed(lambda: g.level_smooth(1, 2, f1, p1), 10)
+            kern["level 1: k_rbt<NS=1,FACES> one sweep per pass"] = {"ms": t / nl, "bytes_per_cell": 48.0, "cells": n1, "sweeps_per_launch": 1}
+            g.set_option(B.MG_OPT_SWEEP_FUSE, 2)
+            t, nl = timed(lambda: g.level_residual_restrict(1, f1, p1), 10)
+            kern["level 1: k_resid_stream<RESTRICT,FACES>"] = {"ms": t / nl, "bytes_per_cell": 41.0, "cells": n1}
+            t, nl = timed(lambda: g.level_prolong_add(1, e2_d, p1), 10)
+            kern["level 1: k_prolong_stream"] = {"ms": t / nl, "bytes_per_cell": 17.0, "cells": n1}
+            del f1, p1, e2_d
         m["kernels"] = kern
 
         # set_density alone
@@ -467,7 +501,7 @@ def assemble_line(args, w, wname, world, m, t_ms, t_e2e_ms, cycles_all, e2e_cycl
     # per-kernel HBM roofline: algorithmic bytes of one launch / event-timed launch duration
     kernels = {}
     for name, k in m.get("kernels", {}).items():
-        ach = k["bytes_per_cell"] * N / (k["ms"] * 1e-3) / 1e9
+        ach = k["bytes_per_cell"] * k.get("cells", N) / (k["ms"] * 1e-3) / 1e9
         kernels[name] = dict(k, achieved_gbs=ach, frac=ach / peak)
     # the cycle uses the two-sweep pass on level 0 from 2^26 cells (mg.cu use_fuse2), the one-sweep pass below
     fused = N >= (1 << 26)
@@ -481,7 +515,8 @@ def assemble_line(args, w, wname, world, m, t_ms, t_e2e_ms, cycles_all, e2e_cycl
                      "its bytes per second are lower than the one-sweep pass's although each sweep is faster: "
                      "the fused pass is bound by shared-memory bandwidth and latency, not by HBM (DESIGN.md 4.1)")
                     if fused else "dominant by share of the V-cycle; one red-black sweep per HBM pass at this size",
-            "per_sweep_equivalent_frac": ((2 if fused else 1) * dom["frac"]) if dom else None,
+            "sweeps_per_pass_times_frac": ((2 if fused else 1) * dom["frac"]) if dom else None,
+            "sweeps_per_pass_times_frac_note": "not a roofline fraction: the 32 B/cell of one pass counted once per fused sweep",
             "kernels": kernels}
     if list(w.n) == [512, 512, 512]:
         roof["traffic"] = NCU_TRAFFIC_512["bytes"]
@@ -493,7 +528,8 @@ def assemble_line(args, w, wname, world, m, t_ms, t_e2e_ms, cycles_all, e2e_cycl
         "config": workload_config(w, wname),
         "solve": {"levels": m["levels"], "cycles_per_solve": m["cycles"], "relres": m["relres"],
                   "l2": f"inputs larger than L2 ({3 * N * 8 / 1e6:.0f} MB resident vs 126 MB)"},
-        "time_to_rtol_ms": m["t_solve_ms"], "set_density_ms": m["t_setrho_ms"],
+        "time_to_rtol_ms": m["t_solve_ms"], "time_to_rtol_samples_ms": m.get("t_solve_samples"),
+        "time_to_rtol_stat": "median of 5 solves", "set_density_ms": m["t_setrho_ms"],
         "f_cycle": m.get("f_cycle"),
         "time_to_rtol_best": (lambda fc: {"ms": min(m["t_solve_ms"], fc["time_to_rtol_ms"]),
                                           "cycle": "F" if fc["time_to_rtol_ms"] < m["t_solve_ms"] else "V"})(m["f_cycle"])
@@ -502,6 +538,7 @@ def assemble_line(args, w, wname, world, m, t_ms, t_e2e_ms, cycles_all, e2e_cycl
                    "launches": m["launches_per_vcycle"],
                    "frac_of_B_sched_roofline": (bs / (peak * 1e9)) / (t_vc_ms * 1e-3),
                    "frac_of_B_sweep_roofline": (bw / (peak * 1e9)) / (t_vc_ms * 1e-3),
+                   "frac_of_B_sched_roofline_at_8000_GBs": (bs / 8000e9) / (t_vc_ms * 1e-3),
                    "B_sched_bytes": bs, "B_sweep_bytes": bw},
         "roofline": roof,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * N * 8, "d2h_bytes_per_step": N * 8,
@@ -556,6 +593,70 @@ def run_cuda(args, w, wname, measure=measure_rank, backend="nccl"):
         dist.destroy_process_group()
 
 
+ONLY_STEPS = ("sweep4", "sweep2", "sweep1", "sweep_restrict", "sweep_norm", "head", "residual", "resid_restrict",
+              "prolong", "vcycle", "fcycle", "solve", "set_density", "box_vcycle", "box_fcycle")
+
+
+def run_only(args, w):
+    """`--only STEP`: launch one step of the cycle `--reps` times on the workload and print its
+    CUDA-event time; the command ncu wraps for the captures under profiles/ (nothing else runs,
+    no JSON line).  `--level L` selects the grid level of the single-step calls, `--kernels`,
+    `--graph`, `--fuse`, `--face-log2` the library options of the same name."""
+    import torch
+
+    import paper_2605_30082_b200 as mgpkg
+    from paper_2605_30082_b200 import binding as B
+
+    step, lev = args.only, args.level
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        bc = (1, 2, 1, 2, 1, 2) if step.startswith("box_") else w.bc
+        g = mgpkg.Multigrid(w.n, w.h, bc, w.nu1, w.nu2, stream=st)
+        g.set_option(B.MG_OPT_KERNELS, args.kernels)
+        g.set_option(B.MG_OPT_GRAPH, args.graph)
+        g.set_option(B.MG_OPT_SWEEP_FUSE, args.fuse)
+        if args.face_log2 is not None:
+            g.set_option(B.MG_OPT_FACE_STREAM_LOG2, args.face_log2)
+        if step in ("fcycle", "box_fcycle"):
+            g.set_cycle_type(B.MG_CYCLE_F)
+        rho = torch.from_numpy(w.rho).cuda()
+        g.set_density(rho)
+        shp = g.level_shape(lev)
+        f = torch.from_numpy(w.rhs).cuda() if lev == 0 else torch.randn(shp, dtype=torch.float64, device="cuda")
+        p = torch.zeros(shp, dtype=torch.float64, device="cuda")
+        e = torch.zeros(g.level_shape(lev + 1), dtype=torch.float64, device="cuda") if lev + 1 < g.num_levels else None
+        calls = {
+            "sweep4": lambda: g.level_smooth(lev, 4, f, p),
+            "sweep2": lambda: g.level_smooth(lev, 2, f, p),
+            "sweep1": lambda: g.level_smooth(lev, 1, f, p),
+            "sweep_restrict": lambda: g.level_smooth_restrict(lev, 1, f, p),
+            "sweep_norm": lambda: g.level_smooth_norm(1, f, p),
+            "head": lambda: g.level_prolong_smooth(lev, 1, e, f, p),
+            "residual": lambda: g.residual(f, p),
+            "resid_restrict": lambda: g.level_residual_restrict(lev, f, p),
+            "prolong": lambda: g.level_prolong_add(lev, e, p),
+            "vcycle": lambda: g.vcycle(f, p),
+            "fcycle": lambda: g.vcycle(f, p),
+            "box_vcycle": lambda: g.vcycle(f, p),
+            "box_fcycle": lambda: g.vcycle(f, p),
+            "solve": lambda: (p.zero_(), g.solve(f, p, w.rtol, 60)),
+            "set_density": lambda: g.set_density(rho),
+        }
+        if step == "head":
+            g.set_option(B.MG_OPT_PROLONG_FUSE, 1)
+        run = calls[step]
+        for _ in range(2):
+            run()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        for _ in range(args.reps):
+            run()
+        e1.record(st)
+        torch.cuda.synchronize()
+        print(f"{step} level {lev} {w.name}: {e0.elapsed_time(e1) / args.reps:.4f} ms per rep")
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -566,11 +667,23 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--full-solve", action="store_true",
                     help="reference arm only: also time the oracle's whole solve once")
-    ap.add_argument("--sequence", type=int, default=0,
+    ap.add_argument("--sequence", type=int, default=4,
                     help="also run a K-step falling-drop sequence (set_density + warm-started solve per step)")
     ap.add_argument("--no-projection", dest="projection", action="store_false",
                     help="skip the projection-step timing (rhs + solve + correct)")
+    ap.add_argument("--only", choices=ONLY_STEPS, default=None,
+                    help="profiling aid: run just this step --reps times (see run_only); prints no JSON line")
+    ap.add_argument("--level", type=int, default=0)
+    ap.add_argument("--reps", type=int, default=5)
+    ap.add_argument("--kernels", type=int, default=1)
+    ap.add_argument("--graph", type=int, default=1)
+    ap.add_argument("--fuse", type=int, default=2)
+    ap.add_argument("--face-log2", type=int, default=None)
     args = ap.parse_args()
+    if args.only:
+        from workloads import make_workload
+        cfg, n = parse_workload(args.workload)
+        return run_only(args, make_workload(cfg, n))
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3
     cmd = spawn_command(args, sys.argv[1:], os.environ) if args.impl == "cuda" else None

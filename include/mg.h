@@ -295,6 +295,14 @@ int mg_level_prolong_smooth(mg_handle *s, int level, int sweeps, const double *e
 int mg_level_restrict_adj(mg_handle *s, int level, const double *r_dev, double *fc_dev);
 int mg_level_prolong_add(mg_handle *s, int level, const double *e_dev, double *p_dev);
 
+/* Verification aid (C5: p = fma(-h2, f, S) * (1.0 / D) with the correctly rounded reciprocal).  The
+ * TMA sweep kernels form 1.0 / D with a branch-free instruction sequence when every a = 0.5/rho
+ * lies in [2^-900, 2^900] (mg_set_density checks), else with the library reciprocal.  This call
+ * evaluates both on n caller values: fast_dev[i] = branch-free sequence, lib_dev[i] = library
+ * reciprocal of d_dev[i]; all device arrays of n doubles; asynchronous on `cuda_stream`.  A test
+ * holds both to the host's 1.0 / d bit for bit over the admitted range (tests/test_gpu_rcp.py). */
+int mg_test_rcp(const double *d_dev, size_t n, double *fast_dev, double *lib_dev, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -47,6 +47,7 @@ SIGNATURES = {
     "mg_project_correct": (C.c_int, [_vp, _dp, C.c_double, _dp, _dp, _dp]),
     "mg_project": (C.c_int, [_vp, _dp, _dp, _dp, C.c_double, _dp, _dp, C.c_double, C.c_int, _ip, _hp]),
     "mg_residual_norm_static": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_double, _ip, _dp, _dp, _dp, _dp, _vp]),
+    "mg_test_rcp": (C.c_int, [_dp, C.c_size_t, _dp, _dp, _vp]),
     "mg_strerror": (C.c_char_p, [C.c_int]),
     "mg_last_cuda_error": (C.c_char_p, []),
     "mg_num_levels": (C.c_int, [_vp]),

@@ -130,11 +130,14 @@ def test_cycles_bit_exact_with_dirichlet_walls(mgmod, uniform, n, bc, cycle_type
     assert g.residual(fd, pg) == pytest.approx(o.residual(f, po), rel=NORM_RTOL)
 
 
-def test_solve_on_the_papers_box(mgmod, uniform):
-    """Drop-film densities in the paper's box: no-slip base, symmetry planes, outflow planes."""
+@pytest.mark.parametrize("size", [64, 256])
+def test_solve_on_the_papers_box(mgmod, uniform, size):
+    """Drop-film densities in the paper's box: no-slip base, symmetry planes, outflow planes;
+    at 64^3 and at config 3's full 256^3 (level 0 runs the TMA kernel with walls, two sweeps per
+    pass from 2^26 cells only, so 256^3 takes the one-sweep passes)."""
     from workloads import make_workload
 
-    w = make_workload(3, 64)
+    w = make_workload(3, size)
     o, g = pair(mgmod, w.n, PAPER_BOX, nu=(w.nu1, w.nu2), rho=w.rho)
     f = w.rhs + 0.1                        # no compatibility condition with a Dirichlet wall
     po = np.zeros(o.shape)

@@ -584,6 +584,18 @@ def test_full_size_config4_bit_exact(mgmod):
     _full_size_cycles(mgmod, 4, 2)
 
 
+@pytest.mark.parametrize("cycle_type", [0, 1], ids=["V", "F"])
+def test_full_size_config4_whole_solve(mgmod, cycle_type):
+    """The timed workload itself (512^3 drop-film, V(3,3), rtol 1e-8), solved to the end with V-cycles
+    (17) and with F-cycles (11) in bench.py's launch configuration (default options: graph replay,
+    two-sweep passes, fused tails): cycle count, every norm of the history to 1e-10, p to 1e-9."""
+    w = make_workload(4)
+    o, g, po, pg, hist = check_solve(mgmod, w, max_cycles=40, cycle_type=cycle_type)
+    assert len(hist) - 1 == (17 if cycle_type == 0 else 11)
+    o.close()
+    g.close()
+
+
 def test_full_size_config5_bit_exact(mgmod):
     """1024^3 (BASELINE configs[4], the largest size): one V(3,3) cycle, every cell.  Needs
     ~60 GB of host memory for the oracle and ~52 GB on the device; skipped on smaller boxes."""
