@@ -85,8 +85,12 @@ enum {
 enum {
     MG_STAT_KERNEL_LAUNCHES = 1,  /* kernels of this library launched so far (graph nodes
                                      counted per replay)                                    */
-    MG_STAT_WORKSPACE_BYTES = 2,  /* device bytes owned by the handle                      */
-    MG_STAT_LAUNCHES_PER_VCYCLE = 3
+    MG_STAT_WORKSPACE_BYTES = 2,  /* device bytes of the workspace (mg_workspace_bytes)     */
+    MG_STAT_LAUNCHES_PER_VCYCLE = 3,
+    MG_STAT_EXTRA_DEVICE_BYTES = 4 /* device bytes the handle holds OUTSIDE the workspace, taken with
+                                     cudaMalloc on first use even by mg_create_in handles and freed by
+                                     mg_destroy: 4 N doubles after the first mg_solve_pcg /
+                                     mg_precondition, 3 N doubles after the first mg_solve_host; 0 before */
 };
 
 /* Bytes of device workspace a solver of this size needs (all levels, all scratch). */
@@ -113,9 +117,10 @@ int mg_create_in(int nx, int ny, int nz, double h, const int bc[3],
  * 2 (a_c + a_c) whose neighbour value is 0; coarse walls are the mean of the four finer wall
  * faces; the prolongation ghost is -e_boundary).  With a Dirichlet wall the system is
  * non-singular: mg_solve checks no compatibility and removes no mean.  Such a solver runs the
- * TMA sweep kernel on level 0 (ghost beyond a Dirichlet wall: a = 3 a_c, p = 0, never updated) and
- * the level-generic kernels for the transfers and the coarser levels down to the persistent
- * coarse CTA; mg_project*, mg_solve_pcg and mg_precondition return MG_EINVAL (the
+ * same kernels as the others: the TMA sweep kernel on level 0 (ghost beyond a Dirichlet wall:
+ * a = 3 a_c, p = 0, never updated) and on the large stored-face levels (plus-wall faces patched into
+ * the staged face tiles), the streaming residual / restriction / prolongation kernels with the wall
+ * logic compiled in, half-sweep launches on the small levels, the persistent coarse CTA; mg_project*, mg_solve_pcg and mg_precondition return MG_EINVAL (the
  * staggered velocity layout has no plus-wall face; the symmetric cycle is defined for periodic
  * and Neumann sides).  Without a Dirichlet side this is mg_create / mg_create_in.  Errors as mg_create. */
 int mg_create6(int nx, int ny, int nz, double h, const int bc6[6], mg_handle **out);
@@ -181,7 +186,8 @@ int mg_solve(mg_handle *s, const double *rhs_dev, double *p_dev, double rtol, in
  * level coarse_sweeps sweeps in each order.  mg_solve_pcg: r = f - A p, z = M r, d = z, then per
  * iteration q = A d, alpha = r.z / d.q, p += alpha d, r -= alpha q, stop when ||r|| <= rtol ||r_0||
  * (r of the recurrence), z = M r, beta = r.z' / r.z, d = z + beta d.  Arguments, return values and
- * hist_host[0..iterations] as mg_solve; four more level-0 arrays are allocated on first use.
+ * hist_host[0..iterations] as mg_solve; four more level-0 arrays (4 N doubles, NOT part of the
+ * workspace or of mg_workspace_bytes; see MG_STAT_EXTRA_DEVICE_BYTES) are allocated with cudaMalloc on first use.
  * MG_EINVAL if nu1 != nu2 or the solver has a Dirichlet side.  On the paper's workloads this
  * iteration needs more work than mg_solve; it is here for completeness. */
 int mg_solve_pcg(mg_handle *s, const double *rhs_dev, double *p_dev, double rtol, int max_iter,

@@ -18,6 +18,7 @@ MG_OPT_FACE_STREAM_LOG2 = 6
 MG_OPT_PROLONG_FUSE = 7
 MG_CYCLE_V, MG_CYCLE_F, MG_CYCLE_W = 0, 1, 2
 MG_STAT_KERNEL_LAUNCHES, MG_STAT_WORKSPACE_BYTES, MG_STAT_LAUNCHES_PER_VCYCLE = 1, 2, 3
+MG_STAT_EXTRA_DEVICE_BYTES = 4
 
 _vp, _dp, _ip = C.c_void_p, C.c_void_p, C.POINTER(C.c_int)   # device pointers travel as integers
 _hp = C.POINTER(C.c_double)

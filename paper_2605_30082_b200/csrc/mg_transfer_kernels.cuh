@@ -17,6 +17,11 @@
 // Neumann wall the neighbour coefficient is taken as -a_c, so that the face a_c + a_nb is
 // exactly +0.0 (C2), and the neighbour value is the (finite) mirror cell.  Coarse levels
 // read their stored minus-face arrays (which hold 0 on a wall).
+// WALLS = true (solvers made by mg_create6 with a Dirichlet side, R24): one boundary type per side.
+// Level 0: a Dirichlet wall face is 2 (a_c + a_c) (C2w) and the value beyond it 0.0; Neumann sides as
+// above.  Stored-face levels: the minus-wall face is entry 0 of the minus-face array as stored, the
+// plus-wall face comes from the level's plus-wall arrays wx, wy, wz (loaded by the boundary threads
+// only), and the value beyond any wall is 0.0 -- the level-generic kernels' rule (mg_common.cuh).
 #pragma once
 #include "mg_common.cuh"
 
@@ -52,7 +57,7 @@ __device__ __forceinline__ double rs_resid(const double b[6], double pxm, double
     return resid_value(ih2, f, S, D, pc);
 }
 
-template <bool CELL, int MODE>
+template <bool CELL, int MODE, bool WALLS = false>
 __global__ void __launch_bounds__(RS_THREADS) k_resid_stream(RsArgs A)
 {
     const Lv &L = A.L;
@@ -72,6 +77,9 @@ __global__ void __launch_bounds__(RS_THREADS) k_resid_stream(RsArgs A)
     const int jm = j0 == 0 ? L.ny - 1 : j0 - 1;
     const int jp = j1 == L.ny - 1 ? 0 : j1 + 1;
     const bool edge_l = lx == 0, edge_r = lx == 31 || x0 + 2 >= L.nx;
+    // WALLS, level 0: which of this thread's walls are Dirichlet
+    const bool dir_xl = WALLS && wall_xl && L.bcm[0] == 2, dir_xr = WALLS && wall_xr && L.bcp[0] == 2;
+    const bool dir_y0 = WALLS && wall_y0 && L.bcm[1] == 2, dir_y1 = WALLS && wall_y1 && L.bcp[1] == 2;
     const size_t plane = (size_t)L.nx * L.ny;
     const size_t row0 = (size_t)L.nx * j0, row1 = (size_t)L.nx * j1, rowm = (size_t)L.nx * jm, rowp = (size_t)L.nx * jp;
 
@@ -119,6 +127,7 @@ __global__ void __launch_bounds__(RS_THREADS) k_resid_stream(RsArgs A)
         load(min(k + 1, kz1 - 1), nxt);
         const size_t oc = plane * (size_t)k;
         const bool wall_z0 = L.bcz && k == 0, wall_z1 = L.bcz && k == L.nz - 1;
+        const bool dir_z0 = WALLS && wall_z0 && L.bcm[2] == 2, dir_z1 = WALLS && wall_z1 && L.bcp[2] == 2;
         Pp[0] = cur.Pp[0]; Pp[1] = cur.Pp[1];
         const double2 Pym = cur.Pym, Pyp = cur.Pyp, F0 = cur.F0, F1 = cur.F1;
         double2 Aym, Ayp, Bx[2], By[3];
@@ -156,12 +165,12 @@ __global__ void __launch_bounds__(RS_THREADS) k_resid_stream(RsArgs A)
 #pragma unroll
             for (int xi = 0; xi < 2; ++xi) {
                 const double pc = xi ? Pc[r].y : Pc[r].x;
-                const double pxm = xi ? Pc[r].x : pl[r];
-                const double pxp = xi ? pr[r] : Pc[r].y;
-                const double pym = r ? (xi ? Pc[0].y : Pc[0].x) : (xi ? Pym.y : Pym.x);
-                const double pyp = r ? (xi ? Pyp.y : Pyp.x) : (xi ? Pc[1].y : Pc[1].x);
-                const double pzm = xi ? Pm[r].y : Pm[r].x;
-                const double pzp = xi ? Pp[r].y : Pp[r].x;
+                double pxm = xi ? Pc[r].x : pl[r];
+                double pxp = xi ? pr[r] : Pc[r].y;
+                double pym = r ? (xi ? Pc[0].y : Pc[0].x) : (xi ? Pym.y : Pym.x);
+                double pyp = r ? (xi ? Pyp.y : Pyp.x) : (xi ? Pc[1].y : Pc[1].x);
+                double pzm = xi ? Pm[r].y : Pm[r].x;
+                double pzp = xi ? Pp[r].y : Pp[r].x;
                 const double fv = r ? (xi ? F1.y : F1.x) : (xi ? F0.y : F0.x);
                 double b[6];
                 if (CELL) {
@@ -179,6 +188,15 @@ __global__ void __launch_bounds__(RS_THREADS) k_resid_stream(RsArgs A)
                     b[0] = __dadd_rn(a_c, axm); b[1] = __dadd_rn(a_c, axp);
                     b[2] = __dadd_rn(a_c, aym); b[3] = __dadd_rn(a_c, ayp);
                     b[4] = __dadd_rn(a_c, azm); b[5] = __dadd_rn(a_c, azp);
+                    if (WALLS) {
+                        const double wf = __dmul_rn(2.0, __dadd_rn(a_c, a_c));      // C2w
+                        if (xi == 0 && dir_xl) { b[0] = wf; pxm = 0.0; }
+                        if (xi == 1 && dir_xr) { b[1] = wf; pxp = 0.0; }
+                        if (r == 0 && dir_y0) { b[2] = wf; pym = 0.0; }
+                        if (r == 1 && dir_y1) { b[3] = wf; pyp = 0.0; }
+                        if (dir_z0) { b[4] = wf; pzm = 0.0; }
+                        if (dir_z1) { b[5] = wf; pzp = 0.0; }
+                    }
                 } else {
                     b[0] = xi ? Bx[r].y : Bx[r].x;
                     b[1] = xi ? bxr[r] : Bx[r].y;
@@ -186,6 +204,15 @@ __global__ void __launch_bounds__(RS_THREADS) k_resid_stream(RsArgs A)
                     b[3] = xi ? By[r + 1].y : By[r + 1].x;
                     b[4] = xi ? Bzc[r].y : Bzc[r].x;
                     b[5] = xi ? Bzp[r].y : Bzp[r].x;
+                    if (WALLS) {
+                        const int jr = r ? j1 : j0;
+                        if (xi == 0 && wall_xl) pxm = 0.0;
+                        if (xi == 1 && wall_xr) { b[1] = __ldg(L.wx + (size_t)jr + (size_t)L.ny * (size_t)k); pxp = 0.0; }
+                        if (r == 0 && wall_y0) pym = 0.0;
+                        if (r == 1 && wall_y1) { b[3] = __ldg(L.wy + (size_t)(x0 + xi) + (size_t)L.nx * (size_t)k); pyp = 0.0; }
+                        if (wall_z0) pzm = 0.0;
+                        if (wall_z1) { b[5] = __ldg(L.wz + (size_t)(x0 + xi) + (size_t)L.nx * (size_t)jr); pzp = 0.0; }
+                    }
                 }
                 res[r][xi] = rs_resid(b, pxm, pxp, pym, pyp, pzm, pzp, pc, fv, L.ih2);
             }

@@ -130,6 +130,71 @@ def test_cycles_bit_exact_with_dirichlet_walls(mgmod, uniform, n, bc, cycle_type
     assert g.residual(fd, pg) == pytest.approx(o.residual(f, po), rel=NORM_RTOL)
 
 
+# stored-face levels of a solver with Dirichlet sides in the TMA kernel (k_rbt<.., CELL = false, WALLS>):
+# the plus-wall faces wx, wy are patched into the bx / by tiles, wz replaces the zero-filled bz plane
+FACE_CASES = [
+    ((96, 64, 48), PAPER_BOX),                      # level 1 = 48 x 32 x 24: one tile, all three plus walls Dirichlet
+    ((64, 72, 32), (D, N, D, D, D, N)),
+    ((64, 64, 64), (N, N, N, N, N, D)),
+    ((160, 144, 64), PAPER_BOX),                    # level 1 = 80 x 72 x 32: several tiles in x and y
+    ((144, 160, 96), (P, P, D, D, N, D)),           # periodic images in x along the Dirichlet y walls; level 2 streams too
+    ((128, 136, 64), (D, D, P, P, D, N)),           # periodic images in y along the Dirichlet x walls
+    ((136, 128, 80), (N, D, N, D, P, P)),           # periodic z
+]
+
+
+@pytest.mark.parametrize("n,bc", FACE_CASES)
+@pytest.mark.parametrize("fuse", [1, 3])
+def test_face_levels_streamed_with_dirichlet_walls(mgmod, uniform, n, bc, fuse):
+    from paper_2605_30082_b200 import binding as B
+
+    shp = (n[2], n[1], n[0])
+    o, g = pair(mgmod, n, bc, rho=random_rho(uniform, 161, shp))
+    g.set_option(B.MG_OPT_FACE_STREAM_LOG2, 0)
+    g.set_option(B.MG_OPT_SWEEP_FUSE, fuse)
+    g.set_option(B.MG_OPT_TAIL_FUSION, 2)
+    tested = 0
+    for lvl in range(1, o.num_levels - 1):
+        lshp = o.level_shape(lvl)
+        if min(lshp[1], lshp[2]) < 32 or lshp[0] < 16:
+            break
+        tested += 1
+        f, p0 = uniform(162 + lvl, lshp), uniform(166 + lvl, lshp)
+        fd = dev(f)
+        for sweeps in (1, 2, 3, 4):
+            po = p0.copy()
+            for _ in range(sweeps):
+                o.sweep(f, po, lvl)
+            pg = dev(p0)
+            g.level_smooth(lvl, sweeps, fd, pg)
+            assert np.array_equal(po, host(pg)), f"level {lvl}, {sweeps} sweeps"
+            fc_o = o.restrict(o.residual_level(f, po, lvl), lvl)
+            pg = dev(p0)
+            fc_g = g.level_smooth_restrict(lvl, sweeps, fd, pg)
+            assert np.array_equal(po, host(pg)), f"level {lvl}, {sweeps} sweeps + tail: p"
+            assert np.array_equal(fc_o, host(fc_g)), f"level {lvl}, {sweeps} sweeps + tail: coarse rhs"
+    assert tested >= 1
+
+
+@pytest.mark.parametrize("n,bc", FACE_CASES)
+@pytest.mark.parametrize("cycle_type", [0, 1], ids=["V", "F"])
+@pytest.mark.parametrize("tails", [1, 2])
+def test_cycles_face_levels_streamed_with_dirichlet_walls(mgmod, uniform, n, bc, cycle_type, tails):
+    from paper_2605_30082_b200 import binding as B
+
+    shp = (n[2], n[1], n[0])
+    o, g = pair(mgmod, n, bc, nu=(3, 3), rho=random_rho(uniform, 171, shp), coarse_sweeps=8, cycle_type=cycle_type)
+    g.set_option(B.MG_OPT_FACE_STREAM_LOG2, 0)
+    g.set_option(B.MG_OPT_TAIL_FUSION, tails)
+    f = uniform(172, shp) + 0.25
+    po, pg, fd = np.zeros(shp), dev(np.zeros(shp)), dev(f)
+    for cyc in range(2):
+        o.vcycle(f, po)
+        g.vcycle(fd, pg)
+        assert np.array_equal(po, host(pg)), f"cycle {cyc}"
+    assert g.residual(fd, pg) == pytest.approx(o.residual(f, po), rel=NORM_RTOL)
+
+
 @pytest.mark.parametrize("size", [64, 256])
 def test_solve_on_the_papers_box(mgmod, uniform, size):
     """Drop-film densities in the paper's box: no-slip base, symmetry planes, outflow planes;

@@ -78,7 +78,10 @@ def test_solve_pcg_matches_the_oracle(mgmod, cfg, n):
     po = np.zeros(o.shape)
     so, io, ro, ho = o.solve_pcg(w.rhs, po, w.rtol, 60)
     pg = dev(np.zeros(o.shape))
+    from paper_2605_30082_b200 import binding as B
+    assert g.stat(B.MG_STAT_EXTRA_DEVICE_BYTES) == 0
     sg, ig, rg, hg = g.solve_pcg(dev(w.rhs), pg, w.rtol, 60)
+    assert g.stat(B.MG_STAT_EXTRA_DEVICE_BYTES) == 4 * 8 * w.ncells       # the CG vectors live outside the workspace
     assert so == 0 and (sg, ig) == (so, io)
     hg = np.array(hg)
     assert np.all(np.abs(hg / ho - 1.0) <= HIST_RTOL), (hg, ho)
